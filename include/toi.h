@@ -1,0 +1,181 @@
+/*
+ * toi.h -- C ABI of libtoi: the B200-native (sm_100a) hot path of the Transient-Oriented
+ * Imager (TOI, 2-D mode) of arxiv 2512.06254.
+ *
+ * One call images one time sample ("snapshot") of a Measurement Set:
+ *
+ *   uvw (metres) --SVD plane fit, rotation (section 3.1)-->
+ *   (r1, r2) in wavelengths per channel
+ *   --flags/weights/parallel-hand average (section 3.5)-->
+ *   --gridding, inverse 2-D C2C FFT-->
+ *   --grid correction, crop, 1/(omega Wsum) (Eqs. 7-8)--> dirty image
+ *
+ * All arithmetic runs in CUDA kernels of this library (+ cuFFT for the transform); there is
+ * no CPU fallback.  The paper is silent on the gridding kernel, padding, grid correction and
+ * uniform weighting: the readings taken are listed in DESIGN.md section 3 (G1..G19).
+ *
+ * Conventions
+ *   - every function returns an int status (TOI_OK = 0, errors < 0); nothing throws or aborts;
+ *   - the caller owns every buffer it passes in; the library only reads them;
+ *   - the plan owns every workspace, ring and returned image pointer; nothing is allocated
+ *     after toi_plan_create returns;
+ *   - toi_image_snapshot only ENQUEUES work on a CUDA stream unless `info` is non-NULL;
+ *   - a plan is not thread-safe; different plans are independent;
+ *   - image layout: float32 [N][N] row-major, row j = t2 axis, column i = t1 axis,
+ *     t1(i) = -beta (i - N/2), t2(j) = +beta (j - N/2)  (Eq. 9, 0-based).
+ */
+#ifndef TOI_H_
+#define TOI_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct toi_plan toi_plan; /* opaque */
+
+enum {
+    TOI_OK = 0,
+    TOI_ERR_INVALID_ARG = -1,
+    TOI_ERR_CUDA = -2,
+    TOI_ERR_CUFFT = -3,
+    TOI_ERR_NOMEM = -4,
+    TOI_ERR_DEGENERATE_GEOMETRY = -5, /* collinear baselines or V33 < 1e-6: no visibility plane */
+    TOI_ERR_CALLBACK = -6,
+    TOI_ERR_UNSUPPORTED = -7
+};
+
+enum { TOI_WEIGHT_NATURAL = 0, TOI_WEIGHT_UNIFORM = 1 };
+enum { TOI_MEM_HOST = 0, TOI_MEM_DEVICE = 1 };
+/* gridding kernels: SLIDING is the product; ATOMIC (one thread per sample, 98 global float
+ * atomics) is kept as the ncu comparison point the design replaces. */
+enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1 };
+
+/* The paper's inputs (Measurement Set, image size, cell size) plus the knobs the
+ * paper leaves open.  Zero selects the default of every optional field. */
+typedef struct {
+    int32_t n_baselines;        /* rows of one time sample (cross-correlations only) */
+    int32_t n_channels;         /* CHAN_FREQ length */
+    int32_t n_pols;             /* 1, 2 or 4 correlations per sample */
+    int32_t pol_a, pol_b;       /* the two parallel hands, e.g. (0,3); equal => one hand */
+    const double *chan_freq_hz; /* HOST, [n_channels], copied by toi_plan_create */
+    int32_t image_size;         /* N, even, >= 16 */
+    double cell_size_deg;       /* beta of Eq. 9, degrees */
+    int32_t weighting;          /* TOI_WEIGHT_* */
+    int32_t grid_size;          /* G: 0 -> 2N; even, >= N */
+    int32_t kernel_support;     /* W: 0 -> 7; only 7 is built */
+    int32_t apply_jacobian;     /* 0 -> 1: divide by omega (Eq. 7); 2 -> do not */
+    int32_t input_location;     /* TOI_MEM_*: where toi_image_snapshot's pointers live */
+    int32_t image_ring_depth;   /* 0 -> 5; the image returned stays valid for
+                                   depth-1 further snapshots */
+    int32_t device;             /* CUDA ordinal */
+    int32_t gridder;            /* TOI_GRIDDER_* */
+    int32_t reserved[7];        /* must be 0 */
+} toi_config;
+
+/* Filled when `info` is passed (forces a stream synchronise). */
+typedef struct {
+    double V[9];                /* row-major transform, R = B V^T */
+    double omega;               /* |V11 V22 - V21 V12| (Eq. 8) */
+    double sing[3];             /* singular values of the centred baseline matrix */
+    double wsum;                /* sum_q f_q w_I,q over gridded samples: Eq. 7's N_vis */
+    int64_t n_gridded, n_off_grid, n_flagged;
+    float ms_h2d, ms_planefit, ms_weight, ms_grid, ms_fft, ms_crop, ms_total;
+} toi_snapshot_info;
+
+/* Allocate everything: device input slots, grid ring, image ring, density, cuFFT plan,
+ * correction tables, streams and events.  *out is NULL on failure. */
+int toi_plan_create(const toi_config *cfg, toi_plan **out);
+int toi_plan_destroy(toi_plan *plan);
+
+/*
+ * Image one snapshot.
+ *   uvw_m    float64 [n_baselines][3]  UVW column, metres
+ *   vis      complex64 [n_baselines][n_channels][n_pols]  DATA column (interleaved re, im)
+ *   weights  float32 same shape, or NULL for unit weights (WEIGHT_SPECTRUM)
+ *   flags    uint8 same shape (non-zero = flagged), or NULL (FLAG)
+ *            all four live where cfg.input_location says (host: copied H2D on the stream;
+ *            the host buffers must stay untouched until the stream reaches that point --
+ *            pass `info` or call toi_plan_sync to be sure)
+ *   cuda_stream  a cudaStream_t, or NULL for the plan's own compute stream
+ *   d_image_out  receives a DEVICE pointer to float32 [N][N] inside the plan's image ring
+ *   info     NULL, or filled after synchronising the stream
+ * Returns TOI_ERR_DEGENERATE_GEOMETRY only when it synchronises (info != NULL); otherwise a
+ * degenerate snapshot yields a zero image and the status is reported by toi_plan_sync.
+ * An all-flagged snapshot is TOI_OK with a zero image and wsum = 0.
+ */
+int toi_image_snapshot(toi_plan *plan, const double *uvw_m, const void *vis, const float *weights,
+                       const uint8_t *flags, void *cuda_stream, float **d_image_out,
+                       toi_snapshot_info *info);
+
+/* Wait for everything the plan enqueued; returns the first deferred status since the last
+ * sync (e.g. TOI_ERR_DEGENERATE_GEOMETRY, TOI_ERR_CUDA). */
+int toi_plan_sync(toi_plan *plan);
+
+/* Copy an image of the ring (as returned through d_image_out) to host memory; synchronous. */
+int toi_copy_image_to_host(toi_plan *plan, const float *d_image, float *h_image);
+
+/*
+ * Streamed run (section 4): a depth-2 pinned host ring feeds a depth-2 device
+ * input ring on a copy stream while the compute stream images the previous snapshot; events
+ * chain the slots, the host never waits for compute.
+ *
+ * fill: called for idx = 0, 1, ...; `slot` holds plan-owned PINNED host buffers to write the
+ *   snapshot into.  The callback may instead REPLACE any of the four pointers with its own
+ *   host buffers (pinned for full speed), which must then stay valid and unchanged until
+ *   the fill call for idx + 2 is made or the stream run returns.  weights/flags may be set to NULL.
+ *   Return 0 = ok, 1 = end of data (no snapshot produced), < 0 = error (TOI_ERR_CALLBACK).
+ * sink: called after snapshot idx has been ENQUEUED; d_image is valid in stream order on
+ *   `cuda_stream` and stays valid for ring_depth-1 further snapshots.  info is NULL unless
+ *   the stream was started with want_info != 0 (which synchronises every snapshot).
+ */
+typedef struct {
+    double *uvw_m;
+    void *vis;
+    float *weights;
+    uint8_t *flags;
+} toi_snapshot_buffers;
+
+typedef int (*toi_fill_fn)(void *user, int64_t idx, toi_snapshot_buffers *slot);
+typedef int (*toi_sink_fn)(void *user, int64_t idx, const float *d_image, void *cuda_stream,
+                           const toi_snapshot_info *info);
+
+typedef struct {
+    int64_t n_done;             /* snapshots imaged */
+    double wall_s;              /* host wall clock of the whole run */
+    double gpu_ms;              /* first H2D start -> last image done, CUDA events */
+    double h2d_bytes;           /* total bytes copied host -> device */
+    double h2d_ms_sum;          /* sum of per-snapshot H2D durations (events) */
+    double compute_ms_sum;      /* sum of per-snapshot imaging durations (events) */
+} toi_stream_stats;
+
+int toi_image_stream(toi_plan *plan, int64_t n_snapshots, toi_fill_fn fill, void *fill_user,
+                     toi_sink_fn sink, void *sink_user, int32_t want_info, toi_stream_stats *stats);
+
+/* Human-readable description of the last error of this plan (or of plan creation when plan is
+ * NULL); the string is owned by the library. */
+const char *toi_last_error(const toi_plan *plan);
+
+/* Number of kernel launches (own kernels + cuFFT execs + memsets) the last snapshot enqueued. */
+int toi_last_launch_count(const toi_plan *plan);
+
+/* ---- debug / parity exports: not on the timed path --------------------------------------- */
+/* Inject V (row-major 3x3, host) for subsequent snapshots instead of fitting it; NULL clears.
+ * Index-parity protocol G5 of DESIGN.md. */
+int toi_debug_set_transform(toi_plan *plan, const double *V);
+/* Centre cells of the LAST snapshot's samples, recomputed from its (still resident) uvw:
+ * int32 [n_baselines][n_channels] each, DEVICE pointers. */
+int toi_debug_cell_indices(toi_plan *plan, int32_t *d_iu, int32_t *d_iv);
+/* The LAST snapshot's grid before the FFT, complex64 [G][G], signed cell (kv, ku) stored at
+ * [(kv + G) mod G][(ku + G) mod G]; DEVICE pointer.  Only valid if debug capture was enabled
+ * with toi_debug_keep_grid(plan, 1) before imaging (costs one extra G*G copy per snapshot). */
+int toi_debug_keep_grid(toi_plan *plan, int32_t on);
+int toi_debug_copy_grid(toi_plan *plan, void *d_grid_c64);
+/* Uniform-weighting density of the LAST snapshot, float32 [G][G], same index convention. */
+int toi_debug_copy_density(toi_plan *plan, float *d_density);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TOI_H_ */

@@ -1,0 +1,570 @@
+// toi_plan.cu -- the C ABI of include/toi.h: plan (all memory, cuFFT plan, streams, events),
+// the per-snapshot stage sequence a1..a7 and the streamed pipeline a8.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <chrono>
+#include <new>
+#include <vector>
+
+#include "toi_internal.cuh"
+
+using namespace toi;
+
+namespace {
+
+thread_local char g_create_error[512] = "";
+
+struct DevSlot {
+    double *uvw = nullptr;
+    float2 *vis = nullptr;
+    float *weights = nullptr;
+    uint8_t *flags = nullptr;
+};
+
+enum { EV_START = 0, EV_H2D, EV_FIT, EV_WEIGHT, EV_GRID, EV_FFT, EV_CROP, EV_COUNT };
+
+}  // namespace
+
+struct toi_plan {
+    toi_config cfg;
+    Geometry geo;
+    double S1 = 0, S2 = 0;
+    int n_sms = 148;
+    int apply_jacobian = 1;
+    size_t n_samples = 0, n_elems = 0;
+
+    double *d_s = nullptr, *d_ipsi = nullptr, *d_V_inject = nullptr;
+    SnapState *d_state = nullptr, *h_state = nullptr;
+    DevSlot dev_in[2];
+    toi_snapshot_buffers pin[2] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
+    float2 *d_grid = nullptr, *d_grid_keep = nullptr;
+    float *d_density = nullptr;
+    float *d_images = nullptr;
+    int ring_depth = 5;
+    long long ring_pos = 0;
+    bool inject = false, keep_grid = false;
+    int snap_slot = 0;
+    Inputs last_in = {nullptr, nullptr, nullptr, nullptr};
+
+    cufftHandle fft = 0;
+    bool fft_ok = false;
+    cudaStream_t s_compute = nullptr, s_copy = nullptr, fft_stream = nullptr;
+    cudaEvent_t ev[EV_COUNT] = {};
+    cudaEvent_t ev_h2d_start[2] = {}, ev_h2d_done[2] = {}, ev_c_start[2] = {}, ev_c_done[2] = {}, ev_first = nullptr;
+
+    int deferred = TOI_OK;
+    int last_launches = 0;
+    char err[512] = "";
+};
+
+namespace {
+
+int fail(toi_plan *p, int code, const char *fmt, const char *a = "", const char *b = "")
+{
+    char *dst = p ? p->err : g_create_error;
+    snprintf(dst, 512, fmt, a, b);
+    if (p && p->deferred == TOI_OK) p->deferred = code;
+    return code;
+}
+
+#define CU_TRY(p, expr)                                                                 \
+    do {                                                                                \
+        cudaError_t e_ = (expr);                                                        \
+        if (e_ != cudaSuccess) return fail((p), e_ == cudaErrorMemoryAllocation ? TOI_ERR_NOMEM : TOI_ERR_CUDA, \
+                                           "%s: %s", #expr, cudaGetErrorString(e_));    \
+    } while (0)
+
+// ---- grid-correction table (G11) ------------------------------------------------
+// psi(n) = int_{-W/2}^{W/2} phi(x) cos(2 pi x n / G) dx.  With x = (W/2) sin(theta) the square-root
+// end-point behaviour of phi disappears:
+//   psi(n) = W int_0^{pi/2} exp(beta_k (cos(theta) - 1)) cos(pi W n sin(theta) / G) cos(theta) dtheta,
+// an analytic integrand that Gauss-Legendre integrates to rounding with a few dozen nodes.
+void legendre_rule(int n, std::vector<double> &x, std::vector<double> &w)
+{
+    x.assign(n, 0.0);
+    w.assign(n, 0.0);
+    const double pi = 3.141592653589793238462643383279502884;
+    for (int i = 0; i < n; ++i) {
+        double z = cos(pi * (i + 0.75) / (n + 0.5)), dp = 1.0;
+        for (int it = 0; it < 50; ++it) {
+            double p0 = 1.0, p1 = z;                       // P_0, P_1
+            for (int k = 2; k <= n; ++k) {
+                const double pk = ((2 * k - 1) * z * p1 - (k - 1) * p0) / k;
+                p0 = p1; p1 = pk;
+            }
+            dp = n * (z * p1 - p0) / (z * z - 1.0);        // P_n'(z)
+            const double step = p1 / dp;
+            z -= step;
+            if (fabs(step) < 4e-16) break;
+        }
+        x[i] = z;
+        w[i] = 2.0 / ((1.0 - z * z) * dp * dp);
+    }
+}
+
+void correction_table(int N, int G, std::vector<double> &ipsi)
+{
+    const int nodes = 96;
+    std::vector<double> x, w;
+    legendre_rule(nodes, x, w);
+    const double pi = 3.141592653589793238462643383279502884;
+    const double beta = 2.30 * kW;
+    std::vector<double> ct(nodes), st(nodes), wt(nodes);
+    for (int k = 0; k < nodes; ++k) {
+        const double th = 0.25 * pi * (x[k] + 1.0);        // [0, pi/2]
+        ct[k] = cos(th); st[k] = sin(th);
+        wt[k] = 0.25 * pi * w[k] * kW * exp(beta * (ct[k] - 1.0)) * ct[k];
+    }
+    ipsi.assign(N, 0.0);
+    for (int i = 0; i < N; ++i) {
+        const double f = pi * kW * (double)(i - N / 2) / (double)G;
+        double acc = 0.0;
+        for (int k = 0; k < nodes; ++k) acc += wt[k] * cos(f * st[k]);
+        ipsi[i] = 1.0 / acc;
+    }
+}
+
+int free_plan(toi_plan *p)
+{
+    if (!p) return TOI_OK;
+    cudaSetDevice(p->cfg.device);
+    if (p->s_compute) cudaStreamSynchronize(p->s_compute);
+    if (p->s_copy) cudaStreamSynchronize(p->s_copy);
+    if (p->fft_ok) cufftDestroy(p->fft);
+    cudaFree(p->d_s); cudaFree(p->d_ipsi); cudaFree(p->d_V_inject); cudaFree(p->d_state);
+    cudaFreeHost(p->h_state);
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(p->dev_in[k].uvw); cudaFree(p->dev_in[k].vis);
+        cudaFree(p->dev_in[k].weights); cudaFree(p->dev_in[k].flags);
+        cudaFreeHost(p->pin[k].uvw_m); cudaFreeHost(p->pin[k].vis);
+        cudaFreeHost(p->pin[k].weights); cudaFreeHost(p->pin[k].flags);
+        if (p->ev_h2d_start[k]) cudaEventDestroy(p->ev_h2d_start[k]);
+        if (p->ev_h2d_done[k]) cudaEventDestroy(p->ev_h2d_done[k]);
+        if (p->ev_c_start[k]) cudaEventDestroy(p->ev_c_start[k]);
+        if (p->ev_c_done[k]) cudaEventDestroy(p->ev_c_done[k]);
+    }
+    if (p->ev_first) cudaEventDestroy(p->ev_first);
+    for (int k = 0; k < EV_COUNT; ++k)
+        if (p->ev[k]) cudaEventDestroy(p->ev[k]);
+    cudaFree(p->d_grid); cudaFree(p->d_grid_keep); cudaFree(p->d_density); cudaFree(p->d_images);
+    if (p->s_compute) cudaStreamDestroy(p->s_compute);
+    if (p->s_copy) cudaStreamDestroy(p->s_copy);
+    cudaGetLastError();
+    delete p;
+    return TOI_OK;
+}
+
+// Enqueue stages a1..a7 for the snapshot resident at `in` on `stream`; returns the image slot.
+int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **d_image_out)
+{
+    const Geometry &g = p->geo;
+    const size_t GG = (size_t)g.G * g.G;
+    int launches = 0;
+    if (p->fft_stream != stream) {
+        if (cufftSetStream(p->fft, stream) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
+        p->fft_stream = stream;
+    }
+    // a1-a2: plane fit (also resets the per-snapshot accumulators)
+    launch_planefit(g, in.uvw, p->S1, p->S2, p->inject ? p->d_V_inject : nullptr, p->d_state, stream);
+    ++launches;
+    CU_TRY(p, cudaEventRecord(p->ev[EV_FIT], stream));
+    // a4: uniform-weighting density pass
+    const float *dens = nullptr;
+    if (p->cfg.weighting == TOI_WEIGHT_UNIFORM) {
+        CU_TRY(p, cudaMemsetAsync(p->d_density, 0, GG * sizeof(float), stream));
+        launch_density(g, in, p->d_state, p->d_density, stream);
+        dens = p->d_density;
+        launches += 2;
+    }
+    CU_TRY(p, cudaEventRecord(p->ev[EV_WEIGHT], stream));
+    // a3 + a5: cell indices and gridding onto the zero-filled grid (the zero fill is part of it)
+    CU_TRY(p, cudaMemsetAsync(p->d_grid, 0, GG * sizeof(float2), stream));
+    if (p->cfg.gridder == TOI_GRIDDER_ATOMIC)
+        launch_grid_atomic(g, in, p->d_state, dens, p->d_grid, stream);
+    else
+        launch_grid_sliding(g, in, p->d_state, dens, p->d_grid, p->n_sms, stream);
+    launches += 2;
+    CU_TRY(p, cudaEventRecord(p->ev[EV_GRID], stream));
+    if (p->keep_grid && p->d_grid_keep)
+        CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
+    // a6: inverse C2C FFT in place
+    if (cufftExecC2C(p->fft, (cufftComplex *)p->d_grid, (cufftComplex *)p->d_grid, CUFFT_INVERSE) != CUFFT_SUCCESS)
+        return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
+    ++launches;
+    CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
+    // a7: correction + crop + normalisation into the image ring
+    float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
+    ++p->ring_pos;
+    launch_correct_crop(g, p->d_grid, p->d_ipsi, p->d_state, p->apply_jacobian, img, stream);
+    ++launches;
+    CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
+    CU_TRY(p, cudaGetLastError());
+    p->last_in = in;
+    p->last_launches = launches;
+    if (d_image_out) *d_image_out = img;
+    return TOI_OK;
+}
+
+int h2d_slot(toi_plan *p, int slot, const double *uvw, const void *vis, const float *weights,
+             const uint8_t *flags, cudaStream_t stream, Inputs &in)
+{
+    DevSlot &d = p->dev_in[slot];
+    const Geometry &g = p->geo;
+    CU_TRY(p, cudaMemcpyAsync(d.uvw, uvw, (size_t)g.n_b * 3 * sizeof(double), cudaMemcpyHostToDevice, stream));
+    CU_TRY(p, cudaMemcpyAsync(d.vis, vis, p->n_elems * sizeof(float2), cudaMemcpyHostToDevice, stream));
+    if (weights) CU_TRY(p, cudaMemcpyAsync(d.weights, weights, p->n_elems * sizeof(float), cudaMemcpyHostToDevice, stream));
+    if (flags) CU_TRY(p, cudaMemcpyAsync(d.flags, flags, p->n_elems, cudaMemcpyHostToDevice, stream));
+    in.uvw = d.uvw; in.vis = d.vis;
+    in.weights = weights ? d.weights : nullptr;
+    in.flags = flags ? d.flags : nullptr;
+    return TOI_OK;
+}
+
+size_t input_bytes(const toi_plan *p, bool w, bool f)
+{
+    return (size_t)p->geo.n_b * 24 + p->n_elems * (8 + (w ? 4 : 0) + (f ? 1 : 0));
+}
+
+int read_info(toi_plan *p, cudaStream_t stream, toi_snapshot_info *info, bool had_h2d)
+{
+    CU_TRY(p, cudaMemcpyAsync(p->h_state, p->d_state, sizeof(SnapState), cudaMemcpyDeviceToHost, stream));
+    CU_TRY(p, cudaStreamSynchronize(stream));
+    const SnapState &s = *p->h_state;
+    memcpy(info->V, s.V, sizeof s.V);
+    info->omega = s.omega;
+    memcpy(info->sing, s.sing, sizeof s.sing);
+    info->wsum = s.wsum;
+    info->n_gridded = (int64_t)s.n_gridded;
+    info->n_off_grid = (int64_t)s.n_off_grid;
+    info->n_flagged = (int64_t)s.n_flagged;
+    float ms = 0.0f;
+    info->ms_h2d = 0.0f;
+    if (had_h2d && cudaEventElapsedTime(&ms, p->ev[EV_START], p->ev[EV_H2D]) == cudaSuccess) info->ms_h2d = ms;
+    cudaEventElapsedTime(&info->ms_planefit, p->ev[EV_H2D], p->ev[EV_FIT]);
+    cudaEventElapsedTime(&info->ms_weight, p->ev[EV_FIT], p->ev[EV_WEIGHT]);
+    cudaEventElapsedTime(&info->ms_grid, p->ev[EV_WEIGHT], p->ev[EV_GRID]);
+    cudaEventElapsedTime(&info->ms_fft, p->ev[EV_GRID], p->ev[EV_FFT]);
+    cudaEventElapsedTime(&info->ms_crop, p->ev[EV_FFT], p->ev[EV_CROP]);
+    cudaEventElapsedTime(&info->ms_total, p->ev[EV_START], p->ev[EV_CROP]);
+    cudaGetLastError();
+    if (s.status != TOI_OK)
+        return fail(p, s.status, "degenerate geometry: the snapshot's baselines do not span a plane (or V33 < 1e-6)");
+    return TOI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int toi_plan_create(const toi_config *cfg, toi_plan **out)
+{
+    if (out) *out = nullptr;
+    if (!cfg || !out) return fail(nullptr, TOI_ERR_INVALID_ARG, "cfg and out must be non-NULL");
+    const int N = cfg->image_size;
+    const int G = cfg->grid_size > 0 ? cfg->grid_size : 2 * N;
+    const int W = cfg->kernel_support > 0 ? cfg->kernel_support : kW;
+    if (cfg->n_baselines < 1 || cfg->n_channels < 1) return fail(nullptr, TOI_ERR_INVALID_ARG, "n_baselines and n_channels must be >= 1");
+    if (cfg->n_pols != 1 && cfg->n_pols != 2 && cfg->n_pols != 4) return fail(nullptr, TOI_ERR_INVALID_ARG, "n_pols must be 1, 2 or 4");
+    if (cfg->pol_a < 0 || cfg->pol_a >= cfg->n_pols || cfg->pol_b < 0 || cfg->pol_b >= cfg->n_pols)
+        return fail(nullptr, TOI_ERR_INVALID_ARG, "pol_a/pol_b out of range");
+    if (!cfg->chan_freq_hz) return fail(nullptr, TOI_ERR_INVALID_ARG, "chan_freq_hz is NULL");
+    if (N < 16 || (N & 1)) return fail(nullptr, TOI_ERR_INVALID_ARG, "image_size must be even and >= 16");
+    if ((G & 1) || G < N || G > (1 << 16)) return fail(nullptr, TOI_ERR_INVALID_ARG, "grid_size must be even, >= image_size and <= 65536");
+    if (!(cfg->cell_size_deg > 0.0) || !(cfg->cell_size_deg < 10.0)) return fail(nullptr, TOI_ERR_INVALID_ARG, "cell_size_deg must be in (0, 10)");
+    if (W != kW) return fail(nullptr, TOI_ERR_UNSUPPORTED, "only kernel_support = 7 is built");
+    if (cfg->weighting != TOI_WEIGHT_NATURAL && cfg->weighting != TOI_WEIGHT_UNIFORM) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown weighting");
+    if (cfg->input_location != TOI_MEM_HOST && cfg->input_location != TOI_MEM_DEVICE) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown input_location");
+    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown gridder");
+    if (cfg->image_ring_depth < 0 || cfg->image_ring_depth > 64) return fail(nullptr, TOI_ERR_INVALID_ARG, "image_ring_depth must be in [0, 64]");
+    if (cfg->apply_jacobian < 0 || cfg->apply_jacobian > 2) return fail(nullptr, TOI_ERR_INVALID_ARG, "apply_jacobian must be 0, 1 or 2");
+    for (int k = 0; k < 7; ++k)
+        if (cfg->reserved[k] != 0) return fail(nullptr, TOI_ERR_INVALID_ARG, "reserved fields must be 0");
+    for (int c = 0; c < cfg->n_channels; ++c)
+        if (!(cfg->chan_freq_hz[c] > 0.0) || !isfinite(cfg->chan_freq_hz[c]))
+            return fail(nullptr, TOI_ERR_INVALID_ARG, "chan_freq_hz must be positive and finite");
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, TOI_ERR_CUDA, "no CUDA device: libtoi has no CPU fallback");
+    }
+    if (cfg->device < 0 || cfg->device >= n_dev) return fail(nullptr, TOI_ERR_INVALID_ARG, "device ordinal out of range");
+
+    toi_plan *p = new (std::nothrow) toi_plan();
+    if (!p) return fail(nullptr, TOI_ERR_NOMEM, "out of host memory");
+    p->cfg = *cfg;
+    p->cfg.chan_freq_hz = nullptr;
+    p->cfg.grid_size = G;
+    p->cfg.kernel_support = W;
+    p->apply_jacobian = cfg->apply_jacobian == 2 ? 0 : 1;
+    p->ring_depth = cfg->image_ring_depth > 0 ? cfg->image_ring_depth : 5;
+    p->n_samples = (size_t)cfg->n_baselines * cfg->n_channels;
+    p->n_elems = p->n_samples * cfg->n_pols;
+
+#define CREATE_TRY(expr)                                                                             \
+    do {                                                                                             \
+        cudaError_t e_ = (expr);                                                                     \
+        if (e_ != cudaSuccess) {                                                                     \
+            int rc_ = fail(nullptr, e_ == cudaErrorMemoryAllocation ? TOI_ERR_NOMEM : TOI_ERR_CUDA, \
+                           "%s: %s", #expr, cudaGetErrorString(e_));                                 \
+            free_plan(p);                                                                            \
+            return rc_;                                                                              \
+        }                                                                                            \
+    } while (0)
+
+    CREATE_TRY(cudaSetDevice(cfg->device));
+    cudaDeviceProp prop;
+    CREATE_TRY(cudaGetDeviceProperties(&prop, cfg->device));
+    p->n_sms = prop.multiProcessorCount;
+
+    // plan-time scalars (fp64 on the host): s_c = nu_c / c0, kappa = G * beta_rad (normative forms)
+    std::vector<double> s(cfg->n_channels);
+    long double s1 = 0, s2 = 0;
+    for (int c = 0; c < cfg->n_channels; ++c) {
+        s[c] = cfg->chan_freq_hz[c] / 299792458.0;
+        s1 += s[c];
+        s2 += (long double)s[c] * s[c];
+    }
+    p->S1 = (double)s1;
+    p->S2 = (double)s2;
+    Geometry &g = p->geo;
+    g.n_b = cfg->n_baselines; g.n_c = cfg->n_channels; g.n_p = cfg->n_pols;
+    g.pol_a = cfg->pol_a; g.pol_b = cfg->pol_b;
+    g.N = N; g.G = G;
+    g.kappa = (double)G * (cfg->cell_size_deg * (3.14159265358979323846 / 180.0));
+    std::vector<double> ipsi;
+    correction_table(N, G, ipsi);
+
+    const size_t GG = (size_t)G * G;
+    CREATE_TRY(cudaStreamCreateWithFlags(&p->s_compute, cudaStreamNonBlocking));
+    CREATE_TRY(cudaStreamCreateWithFlags(&p->s_copy, cudaStreamNonBlocking));
+    for (int k = 0; k < EV_COUNT; ++k) CREATE_TRY(cudaEventCreate(&p->ev[k]));
+    for (int k = 0; k < 2; ++k) {
+        CREATE_TRY(cudaEventCreate(&p->ev_h2d_start[k]));
+        CREATE_TRY(cudaEventCreate(&p->ev_h2d_done[k]));
+        CREATE_TRY(cudaEventCreate(&p->ev_c_start[k]));
+        CREATE_TRY(cudaEventCreate(&p->ev_c_done[k]));
+    }
+    CREATE_TRY(cudaEventCreate(&p->ev_first));
+    CREATE_TRY(cudaMalloc(&p->d_s, s.size() * sizeof(double)));
+    CREATE_TRY(cudaMemcpy(p->d_s, s.data(), s.size() * sizeof(double), cudaMemcpyHostToDevice));
+    g.s = p->d_s;
+    CREATE_TRY(cudaMalloc(&p->d_ipsi, (size_t)N * sizeof(double)));
+    CREATE_TRY(cudaMemcpy(p->d_ipsi, ipsi.data(), (size_t)N * sizeof(double), cudaMemcpyHostToDevice));
+    CREATE_TRY(cudaMalloc(&p->d_V_inject, 9 * sizeof(double)));
+    CREATE_TRY(cudaMalloc(&p->d_state, sizeof(SnapState)));
+    CREATE_TRY(cudaMemset(p->d_state, 0, sizeof(SnapState)));
+    CREATE_TRY(cudaMallocHost(&p->h_state, sizeof(SnapState)));
+    CREATE_TRY(cudaMalloc(&p->d_grid, GG * sizeof(float2)));
+    if (cfg->weighting == TOI_WEIGHT_UNIFORM) CREATE_TRY(cudaMalloc(&p->d_density, GG * sizeof(float)));
+    CREATE_TRY(cudaMalloc(&p->d_images, (size_t)p->ring_depth * N * N * sizeof(float)));
+    if (cfg->input_location == TOI_MEM_HOST) {
+        for (int k = 0; k < 2; ++k) {                      // device input ring + pinned host ring, depth 2
+            CREATE_TRY(cudaMalloc(&p->dev_in[k].uvw, (size_t)g.n_b * 3 * sizeof(double)));
+            CREATE_TRY(cudaMalloc(&p->dev_in[k].vis, p->n_elems * sizeof(float2)));
+            CREATE_TRY(cudaMalloc(&p->dev_in[k].weights, p->n_elems * sizeof(float)));
+            CREATE_TRY(cudaMalloc(&p->dev_in[k].flags, p->n_elems));
+            CREATE_TRY(cudaMallocHost(&p->pin[k].uvw_m, (size_t)g.n_b * 3 * sizeof(double)));
+            CREATE_TRY(cudaMallocHost(&p->pin[k].vis, p->n_elems * sizeof(float2)));
+            CREATE_TRY(cudaMallocHost(&p->pin[k].weights, p->n_elems * sizeof(float)));
+            CREATE_TRY(cudaMallocHost(&p->pin[k].flags, p->n_elems));
+        }
+    }
+    if (cufftPlan2d(&p->fft, G, G, CUFFT_C2C) != CUFFT_SUCCESS) {
+        fail(nullptr, TOI_ERR_CUFFT, "cufftPlan2d failed");
+        free_plan(p);
+        return TOI_ERR_CUFFT;
+    }
+    p->fft_ok = true;
+    CREATE_TRY(cudaDeviceSynchronize());
+#undef CREATE_TRY
+    *out = p;
+    return TOI_OK;
+}
+
+int toi_plan_destroy(toi_plan *plan) { return free_plan(plan); }
+
+int toi_image_snapshot(toi_plan *p, const double *uvw_m, const void *vis, const float *weights,
+                       const uint8_t *flags, void *cuda_stream, float **d_image_out, toi_snapshot_info *info)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    if (!uvw_m || !vis || !d_image_out) return fail(p, TOI_ERR_INVALID_ARG, "uvw_m, vis and d_image_out must be non-NULL");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    cudaStream_t stream = cuda_stream ? (cudaStream_t)cuda_stream : p->s_compute;
+    Inputs in;
+    CU_TRY(p, cudaEventRecord(p->ev[EV_START], stream));
+    const bool host = p->cfg.input_location == TOI_MEM_HOST;
+    if (host) {
+        p->snap_slot ^= 1;
+        int rc = h2d_slot(p, p->snap_slot, uvw_m, vis, weights, flags, stream, in);
+        if (rc) return rc;
+    } else {
+        in.uvw = uvw_m; in.vis = (const float2 *)vis; in.weights = weights; in.flags = flags;
+    }
+    CU_TRY(p, cudaEventRecord(p->ev[EV_H2D], stream));
+    int rc = enqueue_imaging(p, in, stream, d_image_out);
+    if (rc) return rc;
+    if (info) return read_info(p, stream, info, host);
+    return TOI_OK;
+}
+
+int toi_plan_sync(toi_plan *p)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    CU_TRY(p, cudaDeviceSynchronize());
+    CU_TRY(p, cudaMemcpy(p->h_state, p->d_state, sizeof(SnapState), cudaMemcpyDeviceToHost));
+    int rc = p->deferred;
+    p->deferred = TOI_OK;
+    if (rc == TOI_OK && p->h_state->status != TOI_OK) {
+        rc = p->h_state->status;
+        snprintf(p->err, sizeof p->err, "degenerate geometry in the last snapshot");
+    }
+    return rc;
+}
+
+int toi_copy_image_to_host(toi_plan *p, const float *d_image, float *h_image)
+{
+    if (!p || !d_image || !h_image) return fail(p, TOI_ERR_INVALID_ARG, "NULL argument");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    CU_TRY(p, cudaDeviceSynchronize());
+    CU_TRY(p, cudaMemcpy(h_image, d_image, (size_t)p->geo.N * p->geo.N * sizeof(float), cudaMemcpyDeviceToHost));
+    return TOI_OK;
+}
+
+int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *fill_user, toi_sink_fn sink,
+                     void *sink_user, int32_t want_info, toi_stream_stats *stats)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    if (!fill || n_snapshots < 0) return fail(p, TOI_ERR_INVALID_ARG, "fill callback required, n_snapshots >= 0");
+    if (p->cfg.input_location != TOI_MEM_HOST)
+        return fail(p, TOI_ERR_UNSUPPORTED, "toi_image_stream needs a plan created with input_location = TOI_MEM_HOST");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    toi_stream_stats st;
+    memset(&st, 0, sizeof st);
+    const auto t0 = std::chrono::steady_clock::now();
+    bool used[2] = {false, false};
+    float ms = 0.0f;
+    int rc = TOI_OK;
+    auto harvest = [&](int slot) {     // timings of the snapshot that last used `slot` (already complete)
+        if (cudaEventSynchronize(p->ev_c_done[slot]) != cudaSuccess) return;
+        if (cudaEventElapsedTime(&ms, p->ev_h2d_start[slot], p->ev_h2d_done[slot]) == cudaSuccess) st.h2d_ms_sum += ms;
+        if (cudaEventElapsedTime(&ms, p->ev_c_start[slot], p->ev_c_done[slot]) == cudaSuccess) st.compute_ms_sum += ms;
+    };
+    int64_t n = 0;
+    for (; n < n_snapshots; ++n) {
+        const int slot = (int)(n & 1);
+        if (used[slot]) {
+            // the pinned slot is free once its H2D finished; compute of n-2 is long done
+            CU_TRY(p, cudaEventSynchronize(p->ev_h2d_done[slot]));
+            harvest(slot);
+        }
+        toi_snapshot_buffers b = p->pin[slot];
+        const int frc = fill(fill_user, n, &b);
+        if (frc == 1) break;
+        if (frc < 0) { rc = fail(p, TOI_ERR_CALLBACK, "fill callback failed"); break; }
+        if (!b.uvw_m || !b.vis) { rc = fail(p, TOI_ERR_CALLBACK, "fill callback returned NULL uvw/vis"); break; }
+        // device slot is free once the imaging that read it finished: GPU-side wait only
+        if (used[slot]) CU_TRY(p, cudaStreamWaitEvent(p->s_copy, p->ev_c_done[slot], 0));
+        if (n == 0) CU_TRY(p, cudaEventRecord(p->ev_first, p->s_copy));
+        CU_TRY(p, cudaEventRecord(p->ev_h2d_start[slot], p->s_copy));
+        Inputs in;
+        rc = h2d_slot(p, slot, b.uvw_m, b.vis, b.weights, b.flags, p->s_copy, in);
+        if (rc) break;
+        CU_TRY(p, cudaEventRecord(p->ev_h2d_done[slot], p->s_copy));
+        st.h2d_bytes += (double)input_bytes(p, b.weights != nullptr, b.flags != nullptr);
+        CU_TRY(p, cudaStreamWaitEvent(p->s_compute, p->ev_h2d_done[slot], 0));
+        CU_TRY(p, cudaEventRecord(p->ev_c_start[slot], p->s_compute));
+        CU_TRY(p, cudaEventRecord(p->ev[EV_START], p->s_compute));
+        CU_TRY(p, cudaEventRecord(p->ev[EV_H2D], p->s_compute));
+        float *img = nullptr;
+        rc = enqueue_imaging(p, in, p->s_compute, &img);
+        if (rc) break;
+        CU_TRY(p, cudaEventRecord(p->ev_c_done[slot], p->s_compute));
+        used[slot] = true;
+        toi_snapshot_info info;
+        if (want_info) {
+            rc = read_info(p, p->s_compute, &info, false);
+            if (rc) break;
+        }
+        if (sink) {
+            const int src = sink(sink_user, n, img, (void *)p->s_compute, want_info ? &info : nullptr);
+            if (src < 0) { rc = fail(p, TOI_ERR_CALLBACK, "sink callback failed"); break; }
+        }
+    }
+    cudaStreamSynchronize(p->s_copy);
+    cudaStreamSynchronize(p->s_compute);
+    st.n_done = n;
+    for (int slot = 0; slot < 2; ++slot)
+        if (used[slot]) harvest(slot);
+    if (n > 0) {
+        const int last = (int)((n - 1) & 1);
+        if (cudaEventElapsedTime(&ms, p->ev_first, p->ev_c_done[last]) == cudaSuccess) st.gpu_ms = ms;
+    }
+    cudaGetLastError();
+    st.wall_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    if (stats) *stats = st;
+    if (rc == TOI_OK) {
+        cudaMemcpy(p->h_state, p->d_state, sizeof(SnapState), cudaMemcpyDeviceToHost);
+        if (p->deferred != TOI_OK) { rc = p->deferred; p->deferred = TOI_OK; }
+    }
+    return rc;
+}
+
+const char *toi_last_error(const toi_plan *plan) { return plan ? plan->err : g_create_error; }
+
+int toi_last_launch_count(const toi_plan *plan) { return plan ? plan->last_launches : 0; }
+
+int toi_debug_set_transform(toi_plan *p, const double *V)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    CU_TRY(p, cudaDeviceSynchronize());
+    p->inject = V != nullptr;
+    if (V) CU_TRY(p, cudaMemcpy(p->d_V_inject, V, 9 * sizeof(double), cudaMemcpyHostToDevice));
+    return TOI_OK;
+}
+
+int toi_debug_cell_indices(toi_plan *p, int32_t *d_iu, int32_t *d_iv)
+{
+    if (!p || !d_iu || !d_iv) return fail(p, TOI_ERR_INVALID_ARG, "NULL argument");
+    if (!p->last_in.uvw) return fail(p, TOI_ERR_INVALID_ARG, "no snapshot has been imaged yet");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    CU_TRY(p, cudaDeviceSynchronize());
+    launch_cell_indices(p->geo, p->last_in.uvw, p->d_state, d_iu, d_iv, p->s_compute);
+    CU_TRY(p, cudaGetLastError());
+    CU_TRY(p, cudaStreamSynchronize(p->s_compute));
+    return TOI_OK;
+}
+
+int toi_debug_keep_grid(toi_plan *p, int32_t on)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    if (on && !p->d_grid_keep) CU_TRY(p, cudaMalloc(&p->d_grid_keep, (size_t)p->geo.G * p->geo.G * sizeof(float2)));
+    p->keep_grid = on != 0;
+    return TOI_OK;
+}
+
+int toi_debug_copy_grid(toi_plan *p, void *d_grid_c64)
+{
+    if (!p || !d_grid_c64) return fail(p, TOI_ERR_INVALID_ARG, "NULL argument");
+    if (!p->keep_grid || !p->d_grid_keep) return fail(p, TOI_ERR_INVALID_ARG, "call toi_debug_keep_grid(plan, 1) before imaging");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    CU_TRY(p, cudaDeviceSynchronize());
+    CU_TRY(p, cudaMemcpy(d_grid_c64, p->d_grid_keep, (size_t)p->geo.G * p->geo.G * sizeof(float2), cudaMemcpyDeviceToDevice));
+    return TOI_OK;
+}
+
+int toi_debug_copy_density(toi_plan *p, float *d_density)
+{
+    if (!p || !d_density) return fail(p, TOI_ERR_INVALID_ARG, "NULL argument");
+    if (!p->d_density) return fail(p, TOI_ERR_INVALID_ARG, "plan was not created with uniform weighting");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    CU_TRY(p, cudaDeviceSynchronize());
+    CU_TRY(p, cudaMemcpy(d_density, p->d_density, (size_t)p->geo.G * p->geo.G * sizeof(float), cudaMemcpyDeviceToDevice));
+    return TOI_OK;
+}
+
+}  // extern "C"
