@@ -163,9 +163,10 @@ def toi_plan_sync(plan, allow=()):
     return _check(plan, load().toi_plan_sync(plan), allow)
 
 
-def toi_copy_image_to_host(plan, d_image, image_size):
-    """-> float32 CPU tensor [N, N]."""
-    h = torch.empty((image_size, image_size), dtype=torch.float32)
+def toi_copy_image_to_host(plan, d_image, image_size, out=None):
+    """-> float32 CPU tensor [N, N] (``out`` if given, e.g. a pinned tensor)."""
+    h = torch.empty((image_size, image_size), dtype=torch.float32) if out is None else out
+    assert h.dtype == torch.float32 and h.numel() == image_size * image_size and h.is_contiguous()
     _check(plan, load().toi_copy_image_to_host(plan, C.c_void_p(d_image), C.c_void_p(h.data_ptr())))
     return h
 
