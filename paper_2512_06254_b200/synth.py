@@ -186,14 +186,15 @@ def sky_model(wl: Workload, snapshot: int = 0):
 
 
 def flag_channels(wl: Workload) -> torch.Tensor:
-    """bool [n_chan]: seeded contiguous blocks of 16-128 channels until flag_frac is covered."""
+    """bool [n_chan]: seeded contiguous blocks of 16-128 channels until flag_frac is covered
+    (blocks are capped at flag_frac * n_chan + 1 channels so reduced test shapes are not all-flagged)."""
     flagged = torch.zeros(wl.n_chan, dtype=torch.bool)
     if wl.flag_frac <= 0.0:
         return flagged
     one = torch.zeros(1, dtype=torch.int64)
     k = 0
     while flagged.double().mean().item() < wl.flag_frac and k < 10000:
-        width = min(wl.n_chan, 16 + int(float(hash_uniform(wl.seed, 30, one + k)) * 113))
+        width = min(int(wl.flag_frac * wl.n_chan) + 1, 16 + int(float(hash_uniform(wl.seed, 30, one + k)) * 113))
         start = int(float(hash_uniform(wl.seed, 31, one + k)) * max(1, wl.n_chan - width))
         flagged[start:start + width] = True
         k += 1

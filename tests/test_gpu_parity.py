@@ -46,7 +46,7 @@ def _assert_image(img_gpu, img_orc, what=""):
     err_max = float(np.max(np.abs(img_gpu.astype(np.float64) - img_orc)))
     assert err_l2 <= REL_L2_BAR, "%s rel-L2 %.3e > %.0e" % (what, err_l2, REL_L2_BAR)
     assert err_max <= MAX_ABS_BAR * peak, "%s max-abs %.3e > %.0e * peak %.3e" % (what, err_max, MAX_ABS_BAR, peak)
-    return err_l2, err_max / peak
+    return err_l2, (err_max / peak if peak > 0.0 else 0.0)
 
 
 def _check_all(snap, wl_N, cell, weighting, gridder, pol_a=None, pol_b=None, location=toi.TOI_MEM_DEVICE,
