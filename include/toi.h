@@ -167,8 +167,9 @@ int toi_debug_set_transform(toi_plan *plan, const double *V);
 /* Centre cells of the LAST snapshot's samples, recomputed from its (still resident) uvw:
  * int32 [n_baselines][n_channels] each, DEVICE pointers. */
 int toi_debug_cell_indices(toi_plan *plan, int32_t *d_iu, int32_t *d_iv);
-/* The LAST snapshot's grid before the FFT, complex64 [G][G], signed cell (kv, ku) stored at
- * [(kv + G) mod G][(ku + G) mod G]; DEVICE pointer.  Only valid if debug capture was enabled
+/* The LAST snapshot's grid before the FFT, complex64 [G][G], signed cell (kv, ku) stored CENTRED at
+ * [kv + G/2][ku + G/2] (the layout the gridder writes; the (-1)^(n+m) this gives the FFT output is
+ * undone in the correction kernel); DEVICE pointer.  Only valid if debug capture was enabled
  * with toi_debug_keep_grid(plan, 1) before imaging (costs one extra G*G copy per snapshot). */
 int toi_debug_keep_grid(toi_plan *plan, int32_t on);
 int toi_debug_copy_grid(toi_plan *plan, void *d_grid_c64);

@@ -2,7 +2,8 @@
 // normalisation of Eq. 7:
 //     image[j][i] = Re F[m][n] / (psi(n) psi(m) omega Wsum),  n = i - N/2, m = j - N/2
 // F is cuFFT's unshifted output: pixel offset n lives at array index (n + G) mod G, so the crop is
-// four corner blocks of F and no fftshift pass exists.  1/psi is tabulated in fp64 at plan time
+// four corner blocks of F; the grid went in CENTRED (cell k at index k + G/2), which multiplies F
+// by (-1)^(n+m) (shift theorem) -- undone here by the sign.  No fftshift pass exists.  1/psi is tabulated in fp64 at plan time
 // (G11); omega and Wsum are read from device memory (no host round trip).
 #include "toi_internal.cuh"
 
@@ -20,8 +21,10 @@ k_correct_crop(int N, int G, const float2 *__restrict__ F, const double *__restr
     float out = 0.0f;
     if (st->status == TOI_OK && wsum > 0.0) {
         const double norm = (apply_jacobian ? st->omega : 1.0) * wsum;
-        const float2 f = __ldg(F + (size_t)wrap_index(j - (N >> 1), G) * G + wrap_index(i - (N >> 1), G));
-        out = (float)((double)f.x * (ipsi[i] * ipsi[j] / norm));
+        const int n = i - (N >> 1), m = j - (N >> 1);
+        const float2 f = __ldg(F + (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n));
+        const double v = (double)f.x * (ipsi[i] * ipsi[j] / norm);
+        out = (float)(((n + m) & 1) ? -v : v);
     }
     image[(size_t)j * N + i] = out;
 }

@@ -23,8 +23,8 @@ k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__rest
     int iu = kOffGrid, iv = kOffGrid;
     float w = 0.0f;
     if (c < g.n_c) {
-        double gu, gv;
-        sample_cell(rho1, rho2, g.s[c], g.kappa, gu, gv, iu, iv);
+        float xu, xv;
+        sample_cell(rho1, rho2, g.s[c], g.kappa, iu, iv, xu, xv);
         if (cell_on_grid(iu, iv, g.G)) {
             float wa, wb;
             sample_weights(g, in, ((long long)j * g.n_c + c) * g.n_p, wa, wb);
@@ -46,8 +46,8 @@ k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__rest
     }
     const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
     if (tail && iu != kOffGrid && sum > 0.0f) {
-        atomicAdd(D + (size_t)wrap_index(iv, g.G) * g.G + wrap_index(iu, g.G), sum);
-        atomicAdd(D + (size_t)wrap_index(-iv, g.G) * g.G + wrap_index(-iu, g.G), sum);
+        atomicAdd(D + centre_index(iu, iv, g.G), sum);
+        atomicAdd(D + centre_index(-iu, -iv, g.G), sum);
     }
 }
 

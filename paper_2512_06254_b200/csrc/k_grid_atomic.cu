@@ -18,10 +18,11 @@ k_grid_atomic(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__
     unsigned n_grid = 0, n_off = 0, n_flag = 0;
     if (q < (long long)g.n_b * g.n_c) {
         const int j = (int)(q / g.n_c), c = (int)(q % g.n_c);
-        double rho1, rho2, gu, gv;
+        double rho1, rho2;
         int iu, iv;
+        float xu, xv;
         rotate_baseline(st->V, in.uvw + 3 * j, rho1, rho2);
-        sample_cell(rho1, rho2, g.s[c], g.kappa, gu, gv, iu, iv);
+        sample_cell(rho1, rho2, g.s[c], g.kappa, iu, iv, xu, xv);
         if (!cell_on_grid(iu, iv, g.G)) {
             n_off = 1;
         } else {
@@ -34,19 +35,18 @@ k_grid_atomic(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__
                 n_grid = 1;
                 float2 z = sample_stokes(g, in, q * g.n_p, wa, wb);
                 float f = 1.0f;
-                if (D) f = 1.0f / __ldg(D + (size_t)wrap_index(iv, g.G) * g.G + wrap_index(iu, g.G));
+                if (D) f = 1.0f / __ldg(D + centre_index(iu, iv, g.G));
                 wsum = (double)f * (double)wI;
                 z.x *= f; z.y *= f;
                 float pu[kW], pv[kW];
-                kernel_taps((float)(gu - (double)iu), pu);
-                kernel_taps((float)(gv - (double)iv), pv);
+                kernel_taps2(xu, xv, pu, pv);
 #pragma unroll
                 for (int dv = 0; dv < kW; ++dv) {
-                    float2 *row = grid + (size_t)wrap_index(iv + dv - kH, g.G) * g.G;
+                    float2 *row = grid + centre_index(iu - kH, iv + dv - kH, g.G);
 #pragma unroll
                     for (int du = 0; du < kW; ++du) {
                         const float wt = pu[du] * pv[dv];
-                        float2 *cell = row + wrap_index(iu + du - kH, g.G);
+                        float2 *cell = row + du;
                         atomicAdd(&cell->x, z.x * wt);
                         atomicAdd(&cell->y, z.y * wt);
                     }

@@ -7,19 +7,23 @@
 //    a few hundredths of a cell per channel: consecutive channels share a 7x7 footprint for many
 //    samples and the footprint then slides by ONE cell.  So a group of 7 lanes keeps the whole
 //    7x7 complex footprint in registers (lane = column, 7 row accumulators of packed re/im) and
-//    streams through a strip of consecutive channels.  Per sample each lane does one packed
-//    multiply (z * phi_u[column]) and seven packed FMAs (fma.rn.f32x2 -> FFMA2, new on sm_100).
+//    streams through a strip of consecutive channels.  Per sample each lane issues one FMUL2
+//    (z * phi_u[column]) and seven FFMA2 whose third operand is the scalar phi_v[row] broadcast
+//    to both halves (the .F32 operand form of sm_100's FFMA2) -- 8 issue slots for 49 complex taps.
 //  * When the centre cell moves by one column, only the retiring column (7 cells, one lane) is
 //    flushed; the lane then owns the entering column (columns are owned by absolute column mod 7,
 //    so nothing is shuffled).  When it moves by one row, the retiring row is flushed (one cell
 //    per lane, 56 contiguous bytes) and the row accumulators shift by one register.  Flushes are
-//    vector reductions red.global.add.v2.f32 (one per complex cell).  Per run of ~17 samples that
-//    is 7 reductions instead of 17 * 98 scalar atomics.
+//    vector reductions red.global.add.v2.f32 (one per complex cell) onto the CENTRED grid, whose
+//    addresses are affine in the cell (no wrap-around tests).  Per run of ~17 samples that is 7
+//    reductions instead of 17 * 98 scalar atomics.
 //  * A warp carries four such groups (28 of 32 lanes) on four adjacent strips of one baseline.
 //    All 32 lanes first pre-process 32 samples (fp64 cell index, flags/weights/polarisation
-//    average, 14 kernel taps on the MUFU pipe) into a shared-memory record each; the groups
-//    then consume their 8 records.  Tasks (baseline, block of 4 strips) come from an atomic
-//    queue, so the grid is persistent: 2 CTAs x 8 warps per SM.
+//    average, 14 kernel taps, packed for both axes, square root and exp2 on the MUFU pipe) into
+//    an 80-byte shared-memory record each; the groups then consume their 8 records with
+//    immediate-offset LDS.  The raw inputs of the next batch are requested before the current one
+//    is processed (register prefetch), so HBM latency overlaps a whole batch of arithmetic.
+//    Tasks (baseline, block of 4 strips) come from an atomic queue; the grid is persistent.
 //  * fp32 summation is blocked by construction: register chains are bounded by the time a cell
 //    stays inside a sliding window (tens to a few hundred samples), everything else is summed by
 //    the L2 reduction units.
@@ -28,60 +32,102 @@
 namespace toi {
 namespace {
 
-typedef unsigned long long u64;
-
 constexpr int kGroups = 4;        // 7-lane groups per warp
 constexpr int kBatch = 8;         // samples per group per pre-processing batch (4 * 8 = 32 lanes)
 constexpr int kWarps = 8;         // warps per CTA
-constexpr int kRecQuads = 7;      // record = 7 x 16 B: {zre, zim, iu, iv | pu0..3 | pu4..6,- |
-                                  //                    pv0,pv0,pv1,pv1 | pv2.. | pv4.. | pv6,pv6,-,-}
+constexpr int kRecQuads = 5;      // record = 5 x 16 B: {zre, zim, key, -} {pu0..3} {pu4..6, -} {pv0..3} {pv4..6, -}
+constexpr int kGroupQuads = kBatch * kRecQuads + 2;   // +32 B: groups land on distinct banks
+constexpr int kWarpQuads = kGroups * kGroupQuads;
 constexpr int kModBias = 7 << 20; // makes (x + kModBias) % 7 a mathematical mod for |x| < 2^22
+constexpr unsigned kNoKey = 0x80008000u;   // (iv, iu) = (-32768, -32768): never an on-grid cell
 
-__device__ __forceinline__ u64 pack2(float x, float y)
-{
-    u64 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
-    return r;
-}
-__device__ __forceinline__ float2 unpack2(u64 v)
-{
-    float2 r;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
-    return r;
-}
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
-{
-    u64 d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ u64 mul2(u64 a, u64 b)
-{
-    u64 d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
+// centre cell packed into one word: one compare per sample decides "same footprint as before"
+__device__ __forceinline__ unsigned cell_key(int iu, int iv) { return ((unsigned)iv << 16) | ((unsigned)iu & 0xffffu); }
+__device__ __forceinline__ int key_u(unsigned k) { return (int)(k << 16) >> 16; }
+__device__ __forceinline__ int key_v(unsigned k) { return (int)k >> 16; }
+
 __device__ __forceinline__ void red_cell(float2 *cell, u64 v)
 {
     const float2 f = unpack2(v);
-    if (f.x != 0.0f || f.y != 0.0f)
-        asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cell), "f"(f.x), "f"(f.y) : "memory");
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cell), "f"(f.x), "f"(f.y) : "memory");
 }
 
-__global__ void __launch_bounds__(kWarps * 32, 2)
+// Raw inputs of one sample as they sit in HBM (requested one batch ahead).
+struct Raw {
+    float2 a, b;      // the two parallel hands
+    float wa, wb;
+    unsigned fl;      // bit 0: hand a flagged, bit 1: hand b flagged
+    double s;         // s_c = nu_c / c0
+};
+
+// MODE 4: n_p = 4, hands (0, 3), 16-B aligned weights and 4-B aligned flags -> 2 LDG.64 + LDG.128 + LDG.32
+// MODE 2: n_p = 2, hands (0, 1), 8-B aligned weights, 2-B aligned flags     -> LDG.128 + LDG.64 + LDG.U16
+// MODE 0: anything else, scalar loads
+template <int MODE>
+__device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, long long q, int c, Raw &r)
+{
+    r.s = __ldg(g.s + c);
+    if (MODE == 4) {
+        const float2 *v = in.vis + 4 * q;
+        r.a = __ldg(v);
+        r.b = __ldg(v + 3);
+        r.wa = r.wb = 1.0f;
+        if (in.weights) {
+            const float4 w = __ldg(reinterpret_cast<const float4 *>(in.weights) + q);
+            r.wa = w.x; r.wb = w.w;
+        }
+        r.fl = 0u;
+        if (in.flags) {
+            const unsigned f = __ldg(reinterpret_cast<const unsigned *>(in.flags) + q);
+            r.fl = ((f & 0xffu) ? 1u : 0u) | ((f >> 24) ? 2u : 0u);
+        }
+    } else if (MODE == 2) {
+        const float4 v = __ldg(reinterpret_cast<const float4 *>(in.vis) + q);
+        r.a = make_float2(v.x, v.y);
+        r.b = make_float2(v.z, v.w);
+        r.wa = r.wb = 1.0f;
+        if (in.weights) {
+            const float2 w = __ldg(reinterpret_cast<const float2 *>(in.weights) + q);
+            r.wa = w.x; r.wb = w.y;
+        }
+        r.fl = 0u;
+        if (in.flags) {
+            const unsigned f = __ldg(reinterpret_cast<const unsigned short *>(in.flags) + q);
+            r.fl = ((f & 0xffu) ? 1u : 0u) | ((f >> 8) ? 2u : 0u);
+        }
+    } else {
+        const long long o = q * g.n_p;
+        r.a = __ldg(in.vis + o + g.pol_a);
+        r.b = __ldg(in.vis + o + g.pol_b);
+        r.wa = r.wb = 1.0f;
+        if (in.weights) { r.wa = __ldg(in.weights + o + g.pol_a); r.wb = __ldg(in.weights + o + g.pol_b); }
+        r.fl = 0u;
+        if (in.flags) r.fl = (__ldg(in.flags + o + g.pol_a) ? 1u : 0u) | (__ldg(in.flags + o + g.pol_b) ? 2u : 0u);
+        if (g.pol_b == g.pol_a) r.fl |= 2u;     // single hand: b never contributes
+    }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(kWarps * 32, 3)
 k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__restrict__ D,
                float2 *__restrict__ grid, int strip_len, int tasks_per_row, unsigned n_tasks)
 {
-    __shared__ float4 s_rec[kWarps][32 * kRecQuads];
+    __shared__ uint4 s_rec[kWarps * kWarpQuads];
     if (st->status != TOI_OK) return;
     const int lane = threadIdx.x & 31;
-    float4 *rec = s_rec[threadIdx.x >> 5];
+    uint4 *rec = s_rec + (threadIdx.x >> 5) * kWarpQuads;
 
-    // roles: every lane pre-processes one sample per batch; lanes 0..27 accumulate
-    const int pre_k = lane >> 2, pre_g = lane & 3;
+    // roles: every lane pre-processes one sample per batch (strip pre_g, channel pre_k of the
+    // batch: 8 consecutive samples per strip = 256 contiguous bytes of visibilities); lanes 0..27
+    // accumulate (group grp = strip, lane m of the group = one column of the footprint)
+    const int pre_g = lane >> 3, pre_k = lane & 7;
+    uint4 *my_rec = rec + pre_g * kGroupQuads + pre_k * kRecQuads;
     const bool acc_lane = lane < 7 * kGroups;
-    const int grp = lane / 7, m = lane - 7 * grp;
+    const int grp = acc_lane ? lane / 7 : 0, m = lane - 7 * grp;
+    const uint4 *rg = rec + grp * kGroupQuads;
     const int G = g.G;
+    float2 *const gc = grid + centre_index(0, 0, G);         // cell (0, 0)
+    const float *const Dc = D ? D + centre_index(0, 0, G) : nullptr;
 
     double wsum = 0.0;
     unsigned n_grid = 0, n_off = 0, n_flag = 0;
@@ -95,80 +141,89 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
         const int c_task = (int)(task % (unsigned)tasks_per_row) * (kGroups * strip_len);
         double rho1, rho2;
         rotate_baseline(st->V, in.uvw + 3 * j, rho1, rho2);
-        const int c_lo = c_task + pre_g * strip_len;
-        const int c_hi = min(c_lo + strip_len, g.n_c);
-        const int c_end = min(c_task + kGroups * strip_len, g.n_c);   // of the whole task
+        const int c_lo = c_task + pre_g * strip_len + pre_k;      // my channel in batch 0
+        const int c_hi = min(c_task + (pre_g + 1) * strip_len, g.n_c);
+        const long long q_row = (long long)j * g.n_c;
 
         // sliding-window state of my group (uniform across its 7 lanes)
         u64 acc[kW];
 #pragma unroll
         for (int d = 0; d < kW; ++d) acc[d] = 0ull;
-        int cu = kOffGrid, cv = kOffGrid;    // closed window: any real cell mismatches
+        unsigned ckey = kNoKey;              // closed window
+        int cu = 0, cv = 0;
         int mydu = 0;                        // which tap column of the window this lane holds
+        float wpart = 0.0f;
 
-        for (int b = 0; b < strip_len && c_task + b < c_end; b += kBatch) {
+        Raw nxt;
+        nxt.a = nxt.b = make_float2(0.0f, 0.0f); nxt.wa = nxt.wb = 0.0f; nxt.fl = 0u; nxt.s = 0.0;
+        if (c_lo < c_hi) load_raw<MODE>(g, in, q_row + c_lo, c_lo, nxt);
+
+        for (int b = 0; b < strip_len && c_task + b < g.n_c; b += kBatch) {
             // ---------------- pre-process one sample per lane ----------------
             {
-                const int c = c_lo + b + pre_k;
-                float4 q0 = make_float4(0.0f, 0.0f, __int_as_float(kOffGrid), __int_as_float(kOffGrid));
+                const int c = c_lo + b;
+                const Raw cur = nxt;
+                if (c + kBatch < c_hi && b + kBatch < strip_len) load_raw<MODE>(g, in, q_row + c + kBatch, c + kBatch, nxt);
+                uint4 q0 = make_uint4(0u, 0u, kNoKey, 0u);
                 float pu[kW], pv[kW];
 #pragma unroll
                 for (int d = 0; d < kW; ++d) pu[d] = pv[d] = 0.0f;
                 if (c < c_hi) {
-                    double gu, gv;
                     int iu, iv;
-                    sample_cell(rho1, rho2, g.s[c], g.kappa, gu, gv, iu, iv);
+                    float xu, xv;
+                    sample_cell(rho1, rho2, cur.s, g.kappa, iu, iv, xu, xv);
                     if (!cell_on_grid(iu, iv, G)) {
                         ++n_off;
                     } else {
-                        const long long o = ((long long)j * g.n_c + c) * g.n_p;
-                        float wa, wb;
-                        sample_weights(g, in, o, wa, wb);
+                        const float wa = (weight_ok(cur.wa) && !(cur.fl & 1u)) ? cur.wa : 0.0f;
+                        const float wb = (weight_ok(cur.wb) && !(cur.fl & 2u)) ? cur.wb : 0.0f;
                         const float wI = wa + wb;
-                        q0.z = __int_as_float(iu);
-                        q0.w = __int_as_float(iv);
                         if (!(wI > 0.0f)) {
-                            ++n_flag;       // coordinates stay valid, z = 0: the window just slides
+                            ++n_flag;       // contributes nothing: the record stays "no sample"
                         } else {
                             ++n_grid;
-                            float2 z = sample_stokes(g, in, o, wa, wb);
                             float f = 1.0f;
-                            if (D) f = 1.0f / __ldg(D + (size_t)wrap_index(iv, G) * G + wrap_index(iu, G));
-                            wsum += (double)f * (double)wI;
-                            q0.x = z.x * f;
-                            q0.y = z.y * f;
-                            kernel_taps((float)(gu - (double)iu), pu);
-                            kernel_taps((float)(gv - (double)iv), pv);
+                            if (Dc) {
+                                const float dens = __ldg(Dc + ((long long)iv * G + iu));
+                                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(f) : "f"(dens));
+                            }
+                            // z = w_a Vis_a + w_b Vis_b; a zero-weight hand is skipped (its data may be NaN)
+                            float zx = 0.0f, zy = 0.0f;
+                            if (wa > 0.0f) { zx = wa * cur.a.x; zy = wa * cur.a.y; }
+                            if (wb > 0.0f) { zx = fmaf(wb, cur.b.x, zx); zy = fmaf(wb, cur.b.y, zy); }
+                            wpart = fmaf(f, wI, wpart);
+                            q0.x = __float_as_uint(zx * f);
+                            q0.y = __float_as_uint(zy * f);
+                            q0.z = cell_key(iu, iv);
+                            kernel_taps2(xu, xv, pu, pv);
                         }
                     }
                 }
-                float4 *r = rec + lane * kRecQuads;
-                r[0] = q0;
-                r[1] = make_float4(pu[0], pu[1], pu[2], pu[3]);
-                r[2] = make_float4(pu[4], pu[5], pu[6], 0.0f);
-                r[3] = make_float4(pv[0], pv[0], pv[1], pv[1]);
-                r[4] = make_float4(pv[2], pv[2], pv[3], pv[3]);
-                r[5] = make_float4(pv[4], pv[4], pv[5], pv[5]);
-                r[6] = make_float4(pv[6], pv[6], 0.0f, 0.0f);
+                my_rec[0] = q0;
+                my_rec[1] = make_uint4(__float_as_uint(pu[0]), __float_as_uint(pu[1]), __float_as_uint(pu[2]), __float_as_uint(pu[3]));
+                my_rec[2] = make_uint4(__float_as_uint(pu[4]), __float_as_uint(pu[5]), __float_as_uint(pu[6]), 0u);
+                my_rec[3] = make_uint4(__float_as_uint(pv[0]), __float_as_uint(pv[1]), __float_as_uint(pv[2]), __float_as_uint(pv[3]));
+                my_rec[4] = make_uint4(__float_as_uint(pv[4]), __float_as_uint(pv[5]), __float_as_uint(pv[6]), 0u);
             }
             __syncwarp();
-            // ---------------- accumulate: group grp consumes records k*4 + grp ----------------
+            // ---------------- accumulate: group grp consumes its 8 records ----------------
             if (acc_lane) {
+                const float *rpu = reinterpret_cast<const float *>(rg + 1) + mydu;
 #pragma unroll 1
                 for (int k = 0; k < kBatch; ++k) {
-                    const float4 *r = rec + (k * kGroups + grp) * kRecQuads;
-                    const float4 q0 = r[0];
-                    const int iu = __float_as_int(q0.z), iv = __float_as_int(q0.w);
-                    if (iu != cu || iv != cv) {
-                        if (iu == kOffGrid) continue;               // padding / off-grid sample
+                    const uint4 q0 = rg[k * kRecQuads];
+                    // a "no sample" record (padding / off-grid / flagged) has z = 0 and zero taps: it
+                        // falls through the FMAs harmlessly and never moves the window
+                        if (__builtin_expect(q0.z != ckey && q0.z != kNoKey, 0)) {
+                        const int iu = key_u(q0.z), iv = key_v(q0.z);
                         const int du = iu - cu, dv = iv - cv;
-                        if (cu != kOffGrid && du >= -1 && du <= 1 && dv >= -1 && dv <= 1) {
+                        if (ckey != kNoKey && (unsigned)(du + 1) <= 2u && (unsigned)(dv + 1) <= 2u) {
                             if (du != 0) {                          // slide one column
                                 if (mydu == (du > 0 ? 0 : kW - 1)) {
-                                    float2 *col = grid + wrap_index(cu - du * kH, G);
+                                    float2 *p = gc + ((long long)(cv - kH) * G + (cu - du * kH));
 #pragma unroll
                                     for (int d = 0; d < kW; ++d) {
-                                        red_cell(col + (size_t)wrap_index(cv - kH + d, G) * G, acc[d]);
+                                        red_cell(p + (size_t)d * G, acc[d]);
                                         acc[d] = 0ull;
                                     }
                                 }
@@ -177,15 +232,14 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
                                 mydu = mydu < 0 ? kW - 1 : (mydu >= kW ? 0 : mydu);
                             }
                             if (dv != 0) {                          // slide one row
-                                float2 *row = grid + (size_t)wrap_index(cv - dv * kH, G) * G +
-                                              wrap_index(cu - kH + mydu, G);
+                                float2 *p = gc + ((long long)(cv - dv * kH) * G + (cu - kH + mydu));
                                 if (dv > 0) {
-                                    red_cell(row, acc[0]);
+                                    red_cell(p, acc[0]);
 #pragma unroll
                                     for (int d = 0; d < kW - 1; ++d) acc[d] = acc[d + 1];
                                     acc[kW - 1] = 0ull;
                                 } else {
-                                    red_cell(row, acc[kW - 1]);
+                                    red_cell(p, acc[kW - 1]);
 #pragma unroll
                                     for (int d = kW - 1; d > 0; --d) acc[d] = acc[d - 1];
                                     acc[0] = 0ull;
@@ -193,11 +247,11 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
                                 cv += dv;
                             }
                         } else {                                    // first sample, or a jump
-                            if (cu != kOffGrid) {
-                                float2 *col = grid + wrap_index(cu - kH + mydu, G);
+                            if (ckey != kNoKey) {
+                                float2 *p = gc + ((long long)(cv - kH) * G + (cu - kH + mydu));
 #pragma unroll
                                 for (int d = 0; d < kW; ++d) {
-                                    red_cell(col + (size_t)wrap_index(cv - kH + d, G) * G, acc[d]);
+                                    red_cell(p + (size_t)d * G, acc[d]);
                                     acc[d] = 0ull;
                                 }
                             }
@@ -205,30 +259,30 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
                             cv = iv;
                             mydu = (m - cu + kH + kModBias) % kW;   // column (cu-3+mydu) = m (mod 7)
                         }
+                        ckey = q0.z;
+                        rpu = reinterpret_cast<const float *>(rg + 1) + mydu;
                     }
-                    const float pu = reinterpret_cast<const float *>(r + 1)[mydu];
-                    const u64 t = mul2(pack2(q0.x, q0.y), pack2(pu, pu));
-                    const ulonglong2 v01 = *reinterpret_cast<const ulonglong2 *>(r + 3);
-                    const ulonglong2 v23 = *reinterpret_cast<const ulonglong2 *>(r + 4);
-                    const ulonglong2 v45 = *reinterpret_cast<const ulonglong2 *>(r + 5);
-                    const u64 v6 = *reinterpret_cast<const u64 *>(r + 6);
-                    acc[0] = fma2(t, v01.x, acc[0]);
-                    acc[1] = fma2(t, v01.y, acc[1]);
-                    acc[2] = fma2(t, v23.x, acc[2]);
-                    acc[3] = fma2(t, v23.y, acc[3]);
-                    acc[4] = fma2(t, v45.x, acc[4]);
-                    acc[5] = fma2(t, v45.y, acc[5]);
-                    acc[6] = fma2(t, v6, acc[6]);
+                    const float pu = rpu[k * kRecQuads * 4];
+                    const uint4 va = rg[k * kRecQuads + 3], vb = rg[k * kRecQuads + 4];
+                    const u64 t = mul2(pack2(__uint_as_float(q0.x), __uint_as_float(q0.y)), pack2(pu, pu));
+                    fma2_acc(acc[0], t, pack2(__uint_as_float(va.x), __uint_as_float(va.x)));
+                    fma2_acc(acc[1], t, pack2(__uint_as_float(va.y), __uint_as_float(va.y)));
+                    fma2_acc(acc[2], t, pack2(__uint_as_float(va.z), __uint_as_float(va.z)));
+                    fma2_acc(acc[3], t, pack2(__uint_as_float(va.w), __uint_as_float(va.w)));
+                    fma2_acc(acc[4], t, pack2(__uint_as_float(vb.x), __uint_as_float(vb.x)));
+                    fma2_acc(acc[5], t, pack2(__uint_as_float(vb.y), __uint_as_float(vb.y)));
+                    fma2_acc(acc[6], t, pack2(__uint_as_float(vb.z), __uint_as_float(vb.z)));
                 }
             }
             __syncwarp();
         }
         // strip done: flush what is left of the window
-        if (acc_lane && cu != kOffGrid) {
-            float2 *col = grid + wrap_index(cu - kH + mydu, G);
+        if (acc_lane && ckey != kNoKey) {
+            float2 *p = gc + ((long long)(cv - kH) * G + (cu - kH + mydu));
 #pragma unroll
-            for (int d = 0; d < kW; ++d) red_cell(col + (size_t)wrap_index(cv - kH + d, G) * G, acc[d]);
+            for (int d = 0; d < kW; ++d) red_cell(p + (size_t)d * G, acc[d]);
         }
+        wsum += (double)wpart;
     }
 
 #pragma unroll
@@ -257,9 +311,15 @@ void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, con
     const int tasks_per_row = (g.n_c + kGroups * strip - 1) / (kGroups * strip);
     const long long n_tasks = (long long)g.n_b * tasks_per_row;
     long long ctas = (n_tasks + kWarps - 1) / kWarps;
-    if (ctas > 2LL * n_sms) ctas = 2LL * n_sms;   // persistent: 2 CTAs per SM pull from the queue
-    k_grid_sliding<<<(unsigned)ctas, kWarps * 32, 0, stream>>>(g, in, st, d_density, d_grid, strip,
-                                                               tasks_per_row, (unsigned)n_tasks);
+    if (ctas > 3LL * n_sms) ctas = 3LL * n_sms;   // persistent: 3 CTAs per SM pull from the queue
+    const dim3 grid((unsigned)ctas), block(kWarps * 32);
+    const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags, av = (uintptr_t)in.vis;
+    if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
+        k_grid_sliding<4><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks);
+    else if (g.n_p == 2 && g.pol_a == 0 && g.pol_b == 1 && (av & 15) == 0 && (aw & 7) == 0 && (af & 1) == 0)
+        k_grid_sliding<2><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks);
+    else
+        k_grid_sliding<0><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks);
 }
 
 }  // namespace toi

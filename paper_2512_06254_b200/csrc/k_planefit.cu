@@ -129,10 +129,11 @@ __global__ void k_cell_indices(Geometry g, const double *__restrict__ uvw, const
     const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= (long long)g.n_b * g.n_c) return;
     const int j = (int)(q / g.n_c), c = (int)(q % g.n_c);
-    double rho1, rho2, gu, gv;
+    double rho1, rho2;
     int iu, iv;
+    float xu, xv;
     rotate_baseline(st->V, uvw + 3 * j, rho1, rho2);
-    sample_cell(rho1, rho2, g.s[c], g.kappa, gu, gv, iu, iv);
+    sample_cell(rho1, rho2, g.s[c], g.kappa, iu, iv, xu, xv);
     iu_out[q] = iu;
     iv_out[q] = iv;
 }

@@ -51,13 +51,30 @@ __device__ __forceinline__ void rotate_baseline(const double *V, const double *u
     rho2 = __dadd_rn(__dadd_rn(__dmul_rn(V[3], u), __dmul_rn(V[4], v)), __dmul_rn(V[5], w));
 }
 
-__device__ __forceinline__ void sample_cell(double rho1, double rho2, double s_c, double kappa,
-                                            double &gu, double &gv, int &iu, int &iv)
+// floor(y) for |y| < 2^31 without the slow F2I/I2F conversion pipe: adding 2^52 + 2^51 with
+// round-down leaves floor(y) in the low word of the sum (the ulp there is 1), and subtracting the
+// constant again is exact.  Bit-identical to (int)floor(y).
+constexpr double kFloorMagic = 6755399441055744.0;
+__device__ __forceinline__ int floor_to_int(double y, double &fl)
 {
-    gu = -__dmul_rn(__dmul_rn(rho1, s_c), kappa);   // the minus is Eq. 9's x = -beta(...)
-    gv = __dmul_rn(__dmul_rn(rho2, s_c), kappa);
-    iu = (int)floor(__dadd_rn(gu, 0.5));
-    iv = (int)floor(__dadd_rn(gv, 0.5));
+    const double m = __dadd_rd(y, kFloorMagic);
+    fl = __dsub_rn(m, kFloorMagic);
+    return __double2loint(m);
+}
+
+// Normative order (DESIGN.md section 3 step 5): t = rho * s_c; g = -(t * kappa) resp. +(t * kappa);
+// i = floor(g + 1/2).  xu, xv = g - i in [-1/2, 1/2] as fp32 (the sub-cell offsets).
+__device__ __forceinline__ void sample_cell(double rho1, double rho2, double s_c, double kappa,
+                                            int &iu, int &iv, float &xu, float &xv)
+{
+    const double gu = -__dmul_rn(__dmul_rn(rho1, s_c), kappa);   // the minus is Eq. 9's x = -beta(...)
+    const double gv = __dmul_rn(__dmul_rn(rho2, s_c), kappa);
+    double fu, fv;
+    iu = floor_to_int(__dadd_rn(gu, 0.5), fu);
+    iv = floor_to_int(__dadd_rn(gv, 0.5), fv);
+    xu = (float)__dsub_rn(gu, fu);
+    xv = (float)__dsub_rn(gv, fv);
+    if (!(fabs(gu) < 1073741824.0 && fabs(gv) < 1073741824.0)) iu = iv = kOffGrid;   // also NaN
 }
 
 __device__ __forceinline__ bool cell_on_grid(int iu, int iv, int G)
@@ -66,8 +83,14 @@ __device__ __forceinline__ bool cell_on_grid(int iu, int iv, int G)
     return iu >= lo && iu <= hi && iv >= lo && iv <= hi;
 }
 
-// signed cell k in [-G/2, G/2) -> array index (k + G) mod G  (no fftshift pass anywhere)
-__device__ __forceinline__ int wrap_index(int k, int G) { return k < 0 ? k + G : k; }
+// The grid (and the density map) are stored CENTRED: signed cell k in [-G/2, G/2) lives at array
+// index k + G/2, so no address ever wraps while gridding.  cuFFT then sees the input shifted by
+// G/2 on both axes, i.e. its output is (-1)^(n+m) times the transform of the unshifted grid
+// (shift theorem); k_correct_crop applies that sign.  No fftshift pass exists anywhere.
+__device__ __forceinline__ size_t centre_index(int iu, int iv, int G)
+{
+    return (size_t)(iv + (G >> 1)) * (size_t)G + (size_t)(iu + (G >> 1));
+}
 
 // ---- data handling (G12/G13): select, never multiply by zero --------
 __device__ __forceinline__ bool weight_ok(float w) { return w > 0.0f && w <= 3.402823466e+38f; }
@@ -101,21 +124,64 @@ __device__ __forceinline__ float2 sample_stokes(const Geometry &g, const Inputs 
     return z;
 }
 
+// ---- packed fp32 pairs (sm_100a FFMA2 / FMUL2: two fp32 lanes per instruction) ----------------
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pack2(float x, float y)
+{
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
+    return r;
+}
+__device__ __forceinline__ float2 unpack2(u64 v)
+{
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
+{
+    u64 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+// acc += a * b with the accumulator tied to one register pair (keeps ptxas from renaming the
+// accumulators across the branches of the sliding-window loop)
+__device__ __forceinline__ void fma2_acc(u64 &acc, u64 a, u64 b)
+{
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b)
+{
+    u64 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 // Gridding kernel phi(x) = exp(beta_k (sqrt(1 - (2x/W)^2) - 1)) (G9) at the seven taps
-// du = -3..3 of a sample whose sub-cell offset is xoff = g - i in [-0.5, 0.5): tap distance du - xoff.
-__device__ __forceinline__ void kernel_taps(float xoff, float p[kW])
+// du = -3..3 of a sample whose sub-cell offsets are (xu, xv) = g - i in [-0.5, 0.5]: tap distance
+// x = du - xoff, t = 2x/W.  Both axes are evaluated together as packed pairs:
+// 1 - t^2 = (1 - t)(1 + t) is two FFMA2 and one FMUL2, the exponent one FFMA2, and the square
+// root and exp2 go to the MUFU pipe.
+__device__ __forceinline__ void kernel_taps2(float xu, float xv, float pu[kW], float pv[kW])
 {
     constexpr float k2w = 2.0f / kW;
     constexpr float kb2 = kBetaK * 1.4426950408889634f;   // beta_k * log2(e)
+    const u64 X = pack2(xu, xv);
 #pragma unroll
     for (int d = 0; d < kW; ++d) {
-        const float t = fmaf(xoff, -k2w, (float)(d - kH) * k2w);
-        float a = fmaf(-t, t, 1.0f);
-        if (d == kW - 1) a = fmaxf(a, 0.0f);              // only du = +3 can reach |x| = W/2
-        float r;
-        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
-        const float e = fmaf(r, kb2, -kb2);
-        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(p[d]) : "f"(e));
+        const float c = (float)(d - kH) * k2w;            // t = c - k2w * xoff
+        const u64 om = fma2(X, pack2(k2w, k2w), pack2(1.0f - c, 1.0f - c));     // 1 - t
+        const u64 op = fma2(X, pack2(-k2w, -k2w), pack2(1.0f + c, 1.0f + c));   // 1 + t
+        float2 a = unpack2(mul2(om, op));
+        // du = +3 reaches |x| = W/2 at xoff = -1/2 and du = -3 at xoff = +1/2 (an offset just below
+        // 1/2 rounds to 0.5f about once per 10^7 samples): rounding may leave 1 - t^2 at -1e-8
+        if (d == 0 || d == kW - 1) { a.x = fmaxf(a.x, 0.0f); a.y = fmaxf(a.y, 0.0f); }
+        float ru, rv;
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(ru) : "f"(a.x));
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(rv) : "f"(a.y));
+        const float2 e = unpack2(fma2(pack2(ru, rv), pack2(kb2, kb2), pack2(-kb2, -kb2)));
+        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(pu[d]) : "f"(e.x));
+        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(pv[d]) : "f"(e.y));
     }
 }
 

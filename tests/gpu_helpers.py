@@ -50,12 +50,11 @@ class GpuImager:
         return iu.cpu().numpy(), iv.cpu().numpy()
 
     def grid_centred(self):
-        """Pre-FFT grid of the last snapshot, re-ordered to the oracle's centred layout."""
-        g = toi.toi_debug_copy_grid(self.plan, self.G).cpu().numpy()
-        return np.fft.fftshift(g)      # index (k+G)%G -> k+G/2 for even G: a pure permutation
+        """Pre-FFT grid of the last snapshot; libtoi stores it centred (cell k at k + G/2) like the oracle."""
+        return toi.toi_debug_copy_grid(self.plan, self.G).cpu().numpy()
 
     def density_centred(self):
-        return np.fft.fftshift(toi.toi_debug_copy_density(self.plan, self.G).cpu().numpy())
+        return toi.toi_debug_copy_density(self.plan, self.G).cpu().numpy()
 
     def close(self):
         if self.plan is not None:
