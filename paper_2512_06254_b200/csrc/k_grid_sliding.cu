@@ -27,6 +27,8 @@
 //  * fp32 summation is blocked by construction: register chains are bounded by the time a cell
 //    stays inside a sliding window (tens to a few hundred samples), everything else is summed by
 //    the L2 reduction units.
+#include <stdlib.h>
+
 #include "toi_internal.cuh"
 
 namespace toi {
@@ -38,6 +40,10 @@ constexpr int kWarps = 8;         // warps per CTA
 constexpr int kRecQuads = 5;      // record = 5 x 16 B: {zre, zim, key, -} {pu0..3} {pu4..6, -} {pv0..3} {pv4..6, -}
 constexpr int kGroupQuads = kBatch * kRecQuads + 2;   // +32 B: groups land on distinct banks
 constexpr int kWarpQuads = kGroups * kGroupQuads;
+#ifndef KUNROLL
+#define KUNROLL 1
+#endif
+constexpr int kUnroll = KUNROLL;   // records consumed per copy of the accumulate loop body
 constexpr int kModBias = 7 << 20; // makes (x + kModBias) % 7 a mathematical mod for |x| < 2^22
 constexpr unsigned kNoKey = 0x80008000u;   // (iv, iu) = (-32768, -32768): never an on-grid cell
 
@@ -50,6 +56,78 @@ __device__ __forceinline__ void red_cell(float2 *cell, u64 v)
 {
     const float2 f = unpack2(v);
     asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(cell), "f"(f.x), "f"(f.y) : "memory");
+}
+
+// Flush one window column (7 rows, row stride rs bytes, first row at p) and zero it.  One asm
+// block: the accumulators stay in their register pairs and the address walks by one 64-bit add.
+__device__ __forceinline__ void flush_col(u64 (&a)[kW], const char *p, long long rs)
+{
+    asm volatile(
+        "{\n\t.reg .u64 p;\n\t.reg .f32 x, y;\n\t"
+        "mov.u64 p, %7;\n\t"
+        "mov.b64 {x, y}, %0;\n\tred.global.add.v2.f32 [p], {x, y};\n\tadd.s64 p, p, %8;\n\t"
+        "mov.b64 {x, y}, %1;\n\tred.global.add.v2.f32 [p], {x, y};\n\tadd.s64 p, p, %8;\n\t"
+        "mov.b64 {x, y}, %2;\n\tred.global.add.v2.f32 [p], {x, y};\n\tadd.s64 p, p, %8;\n\t"
+        "mov.b64 {x, y}, %3;\n\tred.global.add.v2.f32 [p], {x, y};\n\tadd.s64 p, p, %8;\n\t"
+        "mov.b64 {x, y}, %4;\n\tred.global.add.v2.f32 [p], {x, y};\n\tadd.s64 p, p, %8;\n\t"
+        "mov.b64 {x, y}, %5;\n\tred.global.add.v2.f32 [p], {x, y};\n\tadd.s64 p, p, %8;\n\t"
+        "mov.b64 {x, y}, %6;\n\tred.global.add.v2.f32 [p], {x, y};\n\t"
+        "mov.b64 %0, 0;\n\tmov.b64 %1, 0;\n\tmov.b64 %2, 0;\n\tmov.b64 %3, 0;\n\t"
+        "mov.b64 %4, 0;\n\tmov.b64 %5, 0;\n\tmov.b64 %6, 0;\n\t}"
+        : "+l"(a[0]), "+l"(a[1]), "+l"(a[2]), "+l"(a[3]), "+l"(a[4]), "+l"(a[5]), "+l"(a[6])
+        : "l"(p), "l"(rs)
+        : "memory");
+}
+
+// The window moves by (du, dv), each in {-1, 0, 1}: retire one column (the lane that holds it
+// flushes 7 cells and takes over the entering column) and/or one row (every lane flushes one cell,
+// the row accumulators shift by one register).  p = &grid[cv-3][my column], rs = row stride in
+// bytes, mydu = which tap column this lane holds.  One predicated asm block, so that ptxas keeps
+// the seven accumulators in place instead of copying them around the branches.
+__device__ __forceinline__ void slide_window(u64 (&a)[kW], const char *&p, int &mydu, int du, int dv, long long rs)
+{
+    asm volatile(
+        "{\n\t.reg .pred pc, pu, pd;\n\t.reg .u64 q;\n\t.reg .f32 x, y;\n\t.reg .s32 t;\n\t"
+        "setp.gt.s32 pu, %9, 0;\n\t"
+        "selp.s32 t, 0, 6, pu;\n\t"
+        "setp.ne.s32 pc, %9, 0;\n\t"
+        "setp.eq.and.s32 pc, %8, t, pc;\n\t"
+        "@!pc bra NOCOL;\n\t"
+        "mov.u64 q, %7;\n\t"
+        "mov.b64 {x, y}, %0;\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, %11;\n\t"
+        "mov.b64 {x, y}, %1;\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, %11;\n\t"
+        "mov.b64 {x, y}, %2;\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, %11;\n\t"
+        "mov.b64 {x, y}, %3;\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, %11;\n\t"
+        "mov.b64 {x, y}, %4;\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, %11;\n\t"
+        "mov.b64 {x, y}, %5;\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, %11;\n\t"
+        "mov.b64 {x, y}, %6;\n\tred.global.add.v2.f32 [q], {x, y};\n\t"
+        "mov.b64 %0, 0;\n\tmov.b64 %1, 0;\n\tmov.b64 %2, 0;\n\tmov.b64 %3, 0;\n\t"
+        "mov.b64 %4, 0;\n\tmov.b64 %5, 0;\n\tmov.b64 %6, 0;\n\t"
+        "mad.wide.s32 %7, %9, 56, %7;\n\t"
+        "mad.lo.s32 %8, %9, 7, %8;\n\t"
+        "NOCOL:\n\t"
+        "sub.s32 %8, %8, %9;\n\t"
+        "setp.gt.s32 pu, %10, 0;\n\t"
+        "setp.lt.s32 pd, %10, 0;\n\t"
+        "@!pu bra NOUP;\n\t"
+        "mov.b64 {x, y}, %0;\n\t"
+        "red.global.add.v2.f32 [%7], {x, y};\n\t"
+        "mov.b64 %0, %1;\n\tmov.b64 %1, %2;\n\tmov.b64 %2, %3;\n\tmov.b64 %3, %4;\n\t"
+        "mov.b64 %4, %5;\n\tmov.b64 %5, %6;\n\tmov.b64 %6, 0;\n\t"
+        "add.s64 %7, %7, %11;\n\t"
+        "NOUP:\n\t"
+        "@!pd bra NODN;\n\t"
+        "mad.lo.s64 q, %11, 6, %7;\n\t"
+        "mov.b64 {x, y}, %6;\n\t"
+        "red.global.add.v2.f32 [q], {x, y};\n\t"
+        "mov.b64 %6, %5;\n\tmov.b64 %5, %4;\n\tmov.b64 %4, %3;\n\tmov.b64 %3, %2;\n\t"
+        "mov.b64 %2, %1;\n\tmov.b64 %1, %0;\n\tmov.b64 %0, 0;\n\t"
+        "sub.s64 %7, %7, %11;\n\t"
+        "NODN:\n\t}"
+        : "+l"(a[0]), "+l"(a[1]), "+l"(a[2]), "+l"(a[3]), "+l"(a[4]), "+l"(a[5]), "+l"(a[6]),
+          "+l"(p), "+r"(mydu)
+        : "r"(du), "r"(dv), "l"(rs)
+        : "memory");
 }
 
 // Raw inputs of one sample as they sit in HBM (requested one batch ahead).
@@ -127,6 +205,7 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
     const uint4 *rg = rec + grp * kGroupQuads;
     const int G = g.G;
     float2 *const gc = grid + centre_index(0, 0, G);         // cell (0, 0)
+    const long long rs = (long long)G * 8;                   // row stride in bytes
     const float *const Dc = D ? D + centre_index(0, 0, G) : nullptr;
 
     double wsum = 0.0;
@@ -149,9 +228,9 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
         u64 acc[kW];
 #pragma unroll
         for (int d = 0; d < kW; ++d) acc[d] = 0ull;
-        unsigned ckey = kNoKey;              // closed window
-        int cu = 0, cv = 0;
+        unsigned ckey = kNoKey;              // closed window; else the packed centre cell (cu, cv)
         int mydu = 0;                        // which tap column of the window this lane holds
+        const char *pcol = nullptr;          // &grid[cv - 3][cu - 3 + mydu]: top of my column
         float wpart = 0.0f;
 
         Raw nxt;
@@ -208,62 +287,29 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
             __syncwarp();
             // ---------------- accumulate: group grp consumes its 8 records ----------------
             if (acc_lane) {
-                const float *rpu = reinterpret_cast<const float *>(rg + 1) + mydu;
-#pragma unroll 1
+                const char *const rg0 = reinterpret_cast<const char *>(rg);
+                const char *rpu = rg0 + 16 + 4 * mydu;              // my tap column in record 0
+#pragma unroll kUnroll
                 for (int k = 0; k < kBatch; ++k) {
-                    const uint4 q0 = rg[k * kRecQuads];
+                    const char *const rk = rg0 + k * (kRecQuads * 16);
+                    const uint4 q0 = *reinterpret_cast<const uint4 *>(rk);
                     // a "no sample" record (padding / off-grid / flagged) has z = 0 and zero taps: it
-                        // falls through the FMAs harmlessly and never moves the window
-                        if (__builtin_expect(q0.z != ckey && q0.z != kNoKey, 0)) {
-                        const int iu = key_u(q0.z), iv = key_v(q0.z);
-                        const int du = iu - cu, dv = iv - cv;
+                    // falls through the FMAs harmlessly and never moves the window
+                    if (__builtin_expect(q0.z != ckey && q0.z != kNoKey, 0)) {
+                        const int du = key_u(q0.z) - key_u(ckey), dv = key_v(q0.z) - key_v(ckey);
                         if (ckey != kNoKey && (unsigned)(du + 1) <= 2u && (unsigned)(dv + 1) <= 2u) {
-                            if (du != 0) {                          // slide one column
-                                if (mydu == (du > 0 ? 0 : kW - 1)) {
-                                    float2 *p = gc + ((long long)(cv - kH) * G + (cu - du * kH));
-#pragma unroll
-                                    for (int d = 0; d < kW; ++d) {
-                                        red_cell(p + (size_t)d * G, acc[d]);
-                                        acc[d] = 0ull;
-                                    }
-                                }
-                                cu += du;
-                                mydu -= du;
-                                mydu = mydu < 0 ? kW - 1 : (mydu >= kW ? 0 : mydu);
-                            }
-                            if (dv != 0) {                          // slide one row
-                                float2 *p = gc + ((long long)(cv - dv * kH) * G + (cu - kH + mydu));
-                                if (dv > 0) {
-                                    red_cell(p, acc[0]);
-#pragma unroll
-                                    for (int d = 0; d < kW - 1; ++d) acc[d] = acc[d + 1];
-                                    acc[kW - 1] = 0ull;
-                                } else {
-                                    red_cell(p, acc[kW - 1]);
-#pragma unroll
-                                    for (int d = kW - 1; d > 0; --d) acc[d] = acc[d - 1];
-                                    acc[0] = 0ull;
-                                }
-                                cv += dv;
-                            }
+                            slide_window(acc, pcol, mydu, du, dv, rs);
                         } else {                                    // first sample, or a jump
-                            if (ckey != kNoKey) {
-                                float2 *p = gc + ((long long)(cv - kH) * G + (cu - kH + mydu));
-#pragma unroll
-                                for (int d = 0; d < kW; ++d) {
-                                    red_cell(p + (size_t)d * G, acc[d]);
-                                    acc[d] = 0ull;
-                                }
-                            }
-                            cu = iu;
-                            cv = iv;
+                            if (ckey != kNoKey) flush_col(acc, pcol, rs);
+                            const int cu = key_u(q0.z), cv = key_v(q0.z);
                             mydu = (m - cu + kH + kModBias) % kW;   // column (cu-3+mydu) = m (mod 7)
+                            pcol = reinterpret_cast<const char *>(gc + ((long long)(cv - kH) * G + (cu - kH + mydu)));
                         }
                         ckey = q0.z;
-                        rpu = reinterpret_cast<const float *>(rg + 1) + mydu;
+                        rpu = rg0 + 16 + 4 * mydu;
                     }
-                    const float pu = rpu[k * kRecQuads * 4];
-                    const uint4 va = rg[k * kRecQuads + 3], vb = rg[k * kRecQuads + 4];
+                    const float pu = *reinterpret_cast<const float *>(rpu + k * (kRecQuads * 16));
+                    const uint4 va = *reinterpret_cast<const uint4 *>(rk + 48), vb = *reinterpret_cast<const uint4 *>(rk + 64);
                     const u64 t = mul2(pack2(__uint_as_float(q0.x), __uint_as_float(q0.y)), pack2(pu, pu));
                     fma2_acc(acc[0], t, pack2(__uint_as_float(va.x), __uint_as_float(va.x)));
                     fma2_acc(acc[1], t, pack2(__uint_as_float(va.y), __uint_as_float(va.y)));
@@ -277,11 +323,7 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
             __syncwarp();
         }
         // strip done: flush what is left of the window
-        if (acc_lane && ckey != kNoKey) {
-            float2 *p = gc + ((long long)(cv - kH) * G + (cu - kH + mydu));
-#pragma unroll
-            for (int d = 0; d < kW; ++d) red_cell(p + (size_t)d * G, acc[d]);
-        }
+        if (acc_lane && ckey != kNoKey) flush_col(acc, pcol, rs);
         wsum += (double)wpart;
     }
 
@@ -305,9 +347,16 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
 void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                          float2 *d_grid, int n_sms, cudaStream_t stream)
 {
-    // strip length: a quarter of the row, rounded up to a batch, capped at 256 channels
-    int strip = ((g.n_c + kGroups - 1) / kGroups + kBatch - 1) / kBatch * kBatch;
-    if (strip > 256) strip = 256;
+    // strip length (channels per group per task): long strips amortise the 49-cell flush at a strip
+    // end, short ones balance the persistent grid's tail.  Aim at >= 6 tasks per resident warp,
+    // within [32, 256] channels and a multiple of the 8-sample batch.
+    const long long warps = 3LL * n_sms * kWarps;
+    long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
+    want = want / kBatch * kBatch;
+    int strip = (int)(want < 32 ? 32 : (want > 256 ? 256 : want));
+    const int quarter = ((g.n_c + kGroups - 1) / kGroups + kBatch - 1) / kBatch * kBatch;
+    if (strip > quarter) strip = quarter;
+    if (const char *e = getenv("TOI_STRIP")) strip = atoi(e);   // tuning override (multiple of 8)
     const int tasks_per_row = (g.n_c + kGroups * strip - 1) / (kGroups * strip);
     const long long n_tasks = (long long)g.n_b * tasks_per_row;
     long long ctas = (n_tasks + kWarps - 1) / kWarps;
