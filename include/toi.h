@@ -82,6 +82,8 @@ typedef struct {
     double wsum;                /* sum_q f_q w_I,q over gridded samples: Eq. 7's N_vis */
     int64_t n_gridded, n_off_grid, n_flagged;
     float ms_h2d, ms_planefit, ms_weight, ms_grid, ms_fft, ms_crop, ms_total;
+    float ms_zero;              /* zero fill of the next snapshot's grid (+ density) on the side
+                                   stream; it runs under this snapshot's kernels */
 } toi_snapshot_info;
 
 /* Allocate everything: device input slots, grid ring, image ring, density, cuFFT plan,

@@ -39,8 +39,14 @@ struct toi_plan {
     SnapState *d_state = nullptr, *h_state = nullptr;
     DevSlot dev_in[2];
     toi_snapshot_buffers pin[2] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
-    float2 *d_grid = nullptr, *d_grid_keep = nullptr;
-    float *d_density = nullptr;
+    // grid / density rings of depth 2: while snapshot n is imaged on buffer n & 1, the other buffer
+    // is zero-filled on s_zero for snapshot n + 1 (the fill is DRAM-write bound, the kernels it
+    // runs under are issue bound)
+    float2 *d_grids[2] = {nullptr, nullptr}, *d_grid_keep = nullptr;
+    float *d_dens[2] = {nullptr, nullptr};
+    cudaStream_t s_zero = nullptr;
+    cudaEvent_t ev_zeroed[2] = {}, ev_free[2] = {}, ev_z0 = nullptr, ev_z1 = nullptr;
+    int last_k = 0;
     float *d_images = nullptr;
     int ring_depth = 5;
     long long ring_pos = 0;
@@ -148,7 +154,16 @@ int free_plan(toi_plan *p)
     if (p->ev_first) cudaEventDestroy(p->ev_first);
     for (int k = 0; k < EV_COUNT; ++k)
         if (p->ev[k]) cudaEventDestroy(p->ev[k]);
-    cudaFree(p->d_grid); cudaFree(p->d_grid_keep); cudaFree(p->d_density); cudaFree(p->d_images);
+    if (p->s_zero) cudaStreamSynchronize(p->s_zero);
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(p->d_grids[k]); cudaFree(p->d_dens[k]);
+        if (p->ev_zeroed[k]) cudaEventDestroy(p->ev_zeroed[k]);
+        if (p->ev_free[k]) cudaEventDestroy(p->ev_free[k]);
+    }
+    if (p->ev_z0) cudaEventDestroy(p->ev_z0);
+    if (p->ev_z1) cudaEventDestroy(p->ev_z1);
+    if (p->s_zero) cudaStreamDestroy(p->s_zero);
+    cudaFree(p->d_grid_keep); cudaFree(p->d_images);
     if (p->s_compute) cudaStreamDestroy(p->s_compute);
     if (p->s_copy) cudaStreamDestroy(p->s_copy);
     cudaGetLastError();
@@ -166,40 +181,53 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
         if (cufftSetStream(p->fft, stream) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
         p->fft_stream = stream;
     }
+    // buffers of this snapshot (zero-filled while the previous one was imaged) and, on s_zero, the
+    // zero fill of the other pair for the next snapshot, as soon as its last reader is done
+    const int k = (int)(p->ring_pos & 1), kn = k ^ 1;
+    const bool uniform = p->cfg.weighting == TOI_WEIGHT_UNIFORM;
+    float2 *const grid = p->d_grids[k];
+    CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_zeroed[k], 0));
+    CU_TRY(p, cudaStreamWaitEvent(p->s_zero, p->ev_free[kn], 0));
+    CU_TRY(p, cudaEventRecord(p->ev_z0, p->s_zero));
+    if (uniform) CU_TRY(p, cudaMemsetAsync(p->d_dens[kn], 0, GG * sizeof(float), p->s_zero));
+    CU_TRY(p, cudaMemsetAsync(p->d_grids[kn], 0, GG * sizeof(float2), p->s_zero));
+    CU_TRY(p, cudaEventRecord(p->ev_z1, p->s_zero));
+    CU_TRY(p, cudaEventRecord(p->ev_zeroed[kn], p->s_zero));
+    launches += uniform ? 2 : 1;
     // a1-a2: plane fit (also resets the per-snapshot accumulators)
     launch_planefit(g, in.uvw, p->S1, p->S2, p->inject ? p->d_V_inject : nullptr, p->d_state, stream);
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev[EV_FIT], stream));
     // a4: uniform-weighting density pass
     const float *dens = nullptr;
-    if (p->cfg.weighting == TOI_WEIGHT_UNIFORM) {
-        CU_TRY(p, cudaMemsetAsync(p->d_density, 0, GG * sizeof(float), stream));
-        launch_density(g, in, p->d_state, p->d_density, stream);
-        dens = p->d_density;
-        launches += 2;
+    if (uniform) {
+        launch_density(g, in, p->d_state, p->d_dens[k], stream);
+        dens = p->d_dens[k];
+        ++launches;
     }
     CU_TRY(p, cudaEventRecord(p->ev[EV_WEIGHT], stream));
-    // a3 + a5: cell indices and gridding onto the zero-filled grid (the zero fill is part of it)
-    CU_TRY(p, cudaMemsetAsync(p->d_grid, 0, GG * sizeof(float2), stream));
+    // a3 + a5: cell indices and gridding onto the zero-filled grid
     if (p->cfg.gridder == TOI_GRIDDER_ATOMIC)
-        launch_grid_atomic(g, in, p->d_state, dens, p->d_grid, stream);
+        launch_grid_atomic(g, in, p->d_state, dens, grid, stream);
     else
-        launch_grid_sliding(g, in, p->d_state, dens, p->d_grid, p->n_sms, stream);
-    launches += 2;
+        launch_grid_sliding(g, in, p->d_state, dens, grid, p->n_sms, stream);
+    ++launches;
     CU_TRY(p, cudaEventRecord(p->ev[EV_GRID], stream));
     if (p->keep_grid && p->d_grid_keep)
-        CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
+        CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
     // a6: inverse C2C FFT in place
-    if (cufftExecC2C(p->fft, (cufftComplex *)p->d_grid, (cufftComplex *)p->d_grid, CUFFT_INVERSE) != CUFFT_SUCCESS)
+    if (cufftExecC2C(p->fft, (cufftComplex *)grid, (cufftComplex *)grid, CUFFT_INVERSE) != CUFFT_SUCCESS)
         return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
     // a7: correction + crop + normalisation into the image ring
     float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
     ++p->ring_pos;
-    launch_correct_crop(g, p->d_grid, p->d_ipsi, p->d_state, p->apply_jacobian, img, stream);
+    launch_correct_crop(g, grid, p->d_ipsi, p->d_state, p->apply_jacobian, img, stream);
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
+    CU_TRY(p, cudaEventRecord(p->ev_free[k], stream));
+    p->last_k = k;
     CU_TRY(p, cudaGetLastError());
     p->last_in = in;
     p->last_launches = launches;
@@ -248,6 +276,8 @@ int read_info(toi_plan *p, cudaStream_t stream, toi_snapshot_info *info, bool ha
     cudaEventElapsedTime(&info->ms_fft, p->ev[EV_GRID], p->ev[EV_FFT]);
     cudaEventElapsedTime(&info->ms_crop, p->ev[EV_FFT], p->ev[EV_CROP]);
     cudaEventElapsedTime(&info->ms_total, p->ev[EV_START], p->ev[EV_CROP]);
+    info->ms_zero = 0.0f;
+    if (cudaEventSynchronize(p->ev_z1) == cudaSuccess) cudaEventElapsedTime(&info->ms_zero, p->ev_z0, p->ev_z1);
     cudaGetLastError();
     if (s.status != TOI_OK)
         return fail(p, s.status, "degenerate geometry: the snapshot's baselines do not span a plane (or V33 < 1e-6)");
@@ -356,8 +386,21 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     CREATE_TRY(cudaMalloc(&p->d_state, sizeof(SnapState)));
     CREATE_TRY(cudaMemset(p->d_state, 0, sizeof(SnapState)));
     CREATE_TRY(cudaMallocHost(&p->h_state, sizeof(SnapState)));
-    CREATE_TRY(cudaMalloc(&p->d_grid, GG * sizeof(float2)));
-    if (cfg->weighting == TOI_WEIGHT_UNIFORM) CREATE_TRY(cudaMalloc(&p->d_density, GG * sizeof(float)));
+    CREATE_TRY(cudaStreamCreateWithFlags(&p->s_zero, cudaStreamNonBlocking));
+    CREATE_TRY(cudaEventCreate(&p->ev_z0));
+    CREATE_TRY(cudaEventCreate(&p->ev_z1));
+    for (int k = 0; k < 2; ++k) {
+        CREATE_TRY(cudaMalloc(&p->d_grids[k], GG * sizeof(float2)));
+        CREATE_TRY(cudaMemsetAsync(p->d_grids[k], 0, GG * sizeof(float2), p->s_zero));
+        if (cfg->weighting == TOI_WEIGHT_UNIFORM) {
+            CREATE_TRY(cudaMalloc(&p->d_dens[k], GG * sizeof(float)));
+            CREATE_TRY(cudaMemsetAsync(p->d_dens[k], 0, GG * sizeof(float), p->s_zero));
+        }
+        CREATE_TRY(cudaEventCreateWithFlags(&p->ev_zeroed[k], cudaEventDisableTiming));
+        CREATE_TRY(cudaEventCreateWithFlags(&p->ev_free[k], cudaEventDisableTiming));
+        CREATE_TRY(cudaEventRecord(p->ev_zeroed[k], p->s_zero));
+        CREATE_TRY(cudaEventRecord(p->ev_free[k], p->s_zero));
+    }
     CREATE_TRY(cudaMalloc(&p->d_images, (size_t)p->ring_depth * N * N * sizeof(float)));
     if (cfg->input_location == TOI_MEM_HOST) {
         for (int k = 0; k < 2; ++k) {                      // device input ring + pinned host ring, depth 2
@@ -560,10 +603,10 @@ int toi_debug_copy_grid(toi_plan *p, void *d_grid_c64)
 int toi_debug_copy_density(toi_plan *p, float *d_density)
 {
     if (!p || !d_density) return fail(p, TOI_ERR_INVALID_ARG, "NULL argument");
-    if (!p->d_density) return fail(p, TOI_ERR_INVALID_ARG, "plan was not created with uniform weighting");
+    if (!p->d_dens[0]) return fail(p, TOI_ERR_INVALID_ARG, "plan was not created with uniform weighting");
     CU_TRY(p, cudaSetDevice(p->cfg.device));
     CU_TRY(p, cudaDeviceSynchronize());
-    CU_TRY(p, cudaMemcpy(d_density, p->d_density, (size_t)p->geo.G * p->geo.G * sizeof(float), cudaMemcpyDeviceToDevice));
+    CU_TRY(p, cudaMemcpy(d_density, p->d_dens[p->last_k], (size_t)p->geo.G * p->geo.G * sizeof(float), cudaMemcpyDeviceToDevice));
     return TOI_OK;
 }
 

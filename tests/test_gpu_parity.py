@@ -235,6 +235,27 @@ def test_edge_few_channels(n_chan):
     _check_all(snap, wl.image_size, wl.cell_size_deg, "natural", toi.TOI_GRIDDER_SLIDING)
 
 
+@pytest.mark.parametrize("image_size", [100, 36])
+def test_edge_image_size_not_a_multiple_of_8(image_size):
+    """Even N that is not a multiple of 8: the scalar correction/crop kernel, a non power-of-two FFT."""
+    wl = synth.reduced(synth.CONFIG1, n_ant=8, n_core=8, n_chan=24, image_size=image_size, cell_arcsec=40.0)
+    snap = snapshot_np(wl)
+    _check_all(snap, wl.image_size, wl.cell_size_deg, "natural", toi.TOI_GRIDDER_SLIDING)
+
+
+def test_back_to_back_snapshots_alternate_grid_buffers():
+    """The grid / density buffers are a ring of 2 zero-filled on a side stream: five snapshots in a
+    row (uniform weighting) must all equal the first."""
+    wl = _reduced2(n_ant=12, n_chan=130, image_size=256)
+    snap = snapshot_np(wl)
+    rc, img_o, _, _ = _oracle(snap, wl.image_size, wl.cell_size_deg, "uniform", pol_a=0, pol_b=3)
+    assert rc == 0
+    with GpuImager(snap, wl.image_size, wl.cell_size_deg, "uniform", pol_a=0, pol_b=3) as gi:
+        for _ in range(5):
+            img, _, _ = gi.image()
+            _assert_image(img, img_o, "repeat")
+
+
 def test_edge_non_default_grid_size():
     wl = synth.CONFIG1
     snap = snapshot_np(wl)
