@@ -233,7 +233,7 @@ __device__ __forceinline__ void consume_batch(u64 (&a)[kW], const char *&pcol, i
 struct Raw {
     float2 a, b;      // the two parallel hands
     float wa, wb;
-    unsigned fl;      // raw flag bytes (layout depends on MODE); 0 = nothing flagged
+    unsigned fl;      // raw flag bytes as loaded (layout depends on MODE); decoded at use
     double s;         // s_c = nu_c / c0
 };
 
@@ -255,7 +255,7 @@ __device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, bo
             const float4 w = __ldg(reinterpret_cast<const float4 *>(in.weights) + q);
             r.wa = w.x; r.wb = w.w;
         }
-        if (has_f) r.fl = __ldg(reinterpret_cast<const unsigned *>(in.flags) + q) & 0xff0000ffu;
+        if (has_f) r.fl = __ldg(reinterpret_cast<const unsigned *>(in.flags) + q);
     } else if (MODE == 2) {
         const float4 v = __ldg(reinterpret_cast<const float4 *>(in.vis) + q);
         r.a = make_float2(v.x, v.y);
@@ -264,10 +264,7 @@ __device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, bo
             const float2 w = __ldg(reinterpret_cast<const float2 *>(in.weights) + q);
             r.wa = w.x; r.wb = w.y;
         }
-        if (has_f) {
-            const unsigned f = __ldg(reinterpret_cast<const unsigned short *>(in.flags) + q);
-            r.fl = ((f & 0xff00u) << 16) | (f & 0xffu);
-        }
+        if (has_f) r.fl = __ldg(reinterpret_cast<const unsigned short *>(in.flags) + q);
     } else {
         const long long o = q * g.n_p;
         r.a = __ldg(in.vis + o + g.pol_a);
@@ -356,8 +353,10 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
                         // a flagged sample keeps its own cell as key (z = 0, zero taps): it moves the
                         // window exactly as its unflagged neighbours do and never takes the slow path
                         key = cell_key(iu, iv);
+                        // flag bytes of the two hands inside the raw word (decoded here, not at the load)
+                        constexpr unsigned fmask_b = MODE == 2 ? 0x0000ff00u : 0xff000000u;
                         const float wa = (weight_ok(cur.wa) && !(cur.fl & 0x000000ffu)) ? cur.wa : 0.0f;
-                        const float wb = (weight_ok(cur.wb) && !(cur.fl & 0xff000000u)) ? cur.wb : 0.0f;
+                        const float wb = (weight_ok(cur.wb) && !(cur.fl & fmask_b)) ? cur.wb : 0.0f;
                         wI = wa + wb;
                         if (!(wI > 0.0f)) {
                             ++n_flag;
