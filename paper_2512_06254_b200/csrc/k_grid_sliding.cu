@@ -40,6 +40,7 @@ namespace {
 constexpr int kGroups = 4;        // 7-lane groups per warp
 constexpr int kBatch = 8;         // samples per group per pre-processing batch (4 * 8 = 32 lanes)
 constexpr int kWarps = 8;         // warps per CTA
+constexpr int kCtasPerSm = 3;     // resident CTAs per SM (80 registers per thread; 4 x 64 measured slower)
 constexpr int kRecQuads = 5;      // record = 5 x 16 B: {zre, zim, key, -} {pu0..3} {pu4..6, 0} {pv0..3} {pv4..6, 0}
 constexpr int kGroupQuads = kBatch * kRecQuads + 2;   // +32 B: groups land on distinct banks
 constexpr int kWarpQuads = kGroups * kGroupQuads;
@@ -105,19 +106,17 @@ __device__ __forceinline__ void flush_col(const u64 (&a)[kW], const char *p, lon
     TOI_REC_TEST(K, P, OFF48, OFF64) TOI_REC_HEAD(PN, OFFN) TOI_REC_FMA(P)
 #define TOI_REC_LAST(K, P, OFF48, OFF64) TOI_REC_TEST(K, P, OFF48, OFF64) TOI_REC_FMA(P)
 #define TOI_FLUSH7(A0, A1, A2, A3, A4, A5, A6)                                                        \
-    "mad.wide.u32 q1, %13, 1, %7;\n\tmad.wide.u32 q2, %13, 2, %7;\n\tmad.wide.u32 q3, %13, 3, %7;\n\t" \
-    "mad.wide.u32 q4, %13, 4, %7;\n\tmad.wide.u32 q5, %13, 5, %7;\n\tmad.wide.u32 q6, %13, 6, %7;\n\t" \
-    "mov.b64 {x, y}, " A0 ";\n\tred.global.add.v2.f32 [%7], {x, y};\n\t"                             \
-    "mov.b64 {x, y}, " A1 ";\n\tred.global.add.v2.f32 [q1], {x, y};\n\t"                             \
-    "mov.b64 {x, y}, " A2 ";\n\tred.global.add.v2.f32 [q2], {x, y};\n\t"                             \
-    "mov.b64 {x, y}, " A3 ";\n\tred.global.add.v2.f32 [q3], {x, y};\n\t"                             \
-    "mov.b64 {x, y}, " A4 ";\n\tred.global.add.v2.f32 [q4], {x, y};\n\t"                             \
-    "mov.b64 {x, y}, " A5 ";\n\tred.global.add.v2.f32 [q5], {x, y};\n\t"                             \
-    "mov.b64 {x, y}, " A6 ";\n\tred.global.add.v2.f32 [q6], {x, y};\n\t"                             \
+    "mov.u64 q, %7;\n\tcvt.u64.u32 q1, %13;\n\t"                                                     \
+    "mov.b64 {x, y}, " A0 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
+    "mov.b64 {x, y}, " A1 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
+    "mov.b64 {x, y}, " A2 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
+    "mov.b64 {x, y}, " A3 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
+    "mov.b64 {x, y}, " A4 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
+    "mov.b64 {x, y}, " A5 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
+    "mov.b64 {x, y}, " A6 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\t"                               \
     "mov.b64 " A0 ", {pad, pad};\n\tmov.b64 " A1 ", {pad, pad};\n\tmov.b64 " A2 ", {pad, pad};\n\t"   \
     "mov.b64 " A3 ", {pad, pad};\n\tmov.b64 " A4 ", {pad, pad};\n\tmov.b64 " A5 ", {pad, pad};\n\t"   \
     "mov.b64 " A6 ", {pad, pad};\n\t"
-
 // The window of my group moves to the cell in key<P> (record K):
 //   * "no sample" record (padding / off-grid): nothing moves;
 //   * near move, (du, dv) each in {-1, 0, 1}: the lane that holds the retiring column flushes its 7
@@ -154,19 +153,24 @@ __device__ __forceinline__ void flush_col(const u64 (&a)[kW], const char *p, lon
     "sub.s32 %8, %8, du;\n\t"                                                                         \
     "setp.gt.s32 pu, dv, 0;\n\t"                                                                      \
     "setp.lt.s32 pd, dv, 0;\n\t"                                                                      \
+    "mov.b64 one2, 0x3f8000003f800000;\n\t"            /* rows shift by x * 1 (exact), one FMUL2   */ \
+                                                        /* per row: a plain mov would be coalesced  */ \
+                                                        /* away here and paid for on the fast path  */ \
     "@!pu bra NU" #K ";\n\t"                                                                          \
     "mov.b64 {x, y}, %0;\n\t"                                                                         \
     "red.global.add.v2.f32 [%7], {x, y};\n\t"                                                         \
-    "mov.b64 %0, %1;\n\tmov.b64 %1, %2;\n\tmov.b64 %2, %3;\n\tmov.b64 %3, %4;\n\t"                    \
-    "mov.b64 %4, %5;\n\tmov.b64 %5, %6;\n\tmov.b64 %6, {pad, pad};\n\t"                               \
+    "mul.rn.f32x2 %0, %1, one2;\n\tmul.rn.f32x2 %1, %2, one2;\n\tmul.rn.f32x2 %2, %3, one2;\n\t"      \
+    "mul.rn.f32x2 %3, %4, one2;\n\tmul.rn.f32x2 %4, %5, one2;\n\tmul.rn.f32x2 %5, %6, one2;\n\t"      \
+    "mov.b64 %6, {pad, pad};\n\t"                                                                   \
     "mad.wide.u32 %7, %13, 1, %7;\n\t"                                                                \
     "NU" #K ":\n\t"                                                                                   \
     "@!pd bra F" #K ";\n\t"                                                                           \
     "mad.wide.u32 q, %13, 6, %7;\n\t"                                                                 \
     "mov.b64 {x, y}, %6;\n\t"                                                                         \
     "red.global.add.v2.f32 [q], {x, y};\n\t"                                                          \
-    "mov.b64 %6, %5;\n\tmov.b64 %5, %4;\n\tmov.b64 %4, %3;\n\tmov.b64 %3, %2;\n\t"                    \
-    "mov.b64 %2, %1;\n\tmov.b64 %1, %0;\n\tmov.b64 %0, {pad, pad};\n\t"                               \
+    "mul.rn.f32x2 %6, %5, one2;\n\tmul.rn.f32x2 %5, %4, one2;\n\tmul.rn.f32x2 %4, %3, one2;\n\t"      \
+    "mul.rn.f32x2 %3, %2, one2;\n\tmul.rn.f32x2 %2, %1, one2;\n\tmul.rn.f32x2 %1, %0, one2;\n\t"      \
+    "mov.b64 %0, {pad, pad};\n\t"                                                                   \
     "cvt.u64.u32 q1, %13;\n\tsub.s64 %7, %7, q1;\n\t"                                                 \
     "bra F" #K ";\n\t"                                                                                \
     "O" #K ":\n\t"                                                                                    \
@@ -198,7 +202,7 @@ __device__ __forceinline__ void consume_batch(u64 (&a)[kW], const char *&pcol, i
         "{\n\t"
         ".reg .b32 zx0, zy0, key0, pw0, zx1, zy1, key1, pw1, pad, v0, v1, v2, v3, v4, v5, v6, v7;\n\t"
         ".reg .b32 t1, t2, cu, cv, ou, ov, du, dv;\n\t"
-        ".reg .b64 tt, bb, q, q1, q2, q3, q4, q5, q6;\n\t"
+        ".reg .b64 tt, bb, one2, q, q1;\n\t"
         ".reg .f32 x, y;\n\t"
         ".reg .pred pq, p0, po, pn, pc, pf, pu, pd;\n\t"
         TOI_REC_HEAD(0, 0)
@@ -278,7 +282,7 @@ __device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, bo
 // OPT >= 0: bits kHasW | kHasF | kHasD say at compile time which optional inputs exist;
 // OPT < 0: decided at run time from the pointers.
 template <int MODE, int OPT>
-__global__ void __launch_bounds__(kWarps * 32, 3)
+__global__ void __launch_bounds__(kWarps * 32, kCtasPerSm)
 k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__restrict__ D,
                float2 *__restrict__ grid, int strip_len, int tasks_per_row, unsigned n_tasks)
 {
@@ -433,7 +437,7 @@ void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, con
     // strip length (channels per group per task): long strips amortise the 49-cell flush at a strip
     // end, short ones balance the persistent grid's tail.  Aim at >= 6 tasks per resident warp,
     // within [32, 256] channels and a multiple of the 8-sample batch.
-    const long long warps = 3LL * n_sms * kWarps;
+    const long long warps = (long long)kCtasPerSm * n_sms * kWarps;
     long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
     want = want / kBatch * kBatch;
     int strip = (int)(want < 32 ? 32 : (want > 256 ? 256 : want));
@@ -443,7 +447,7 @@ void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, con
     const int tasks_per_row = (g.n_c + kGroups * strip - 1) / (kGroups * strip);
     const long long n_tasks = (long long)g.n_b * tasks_per_row;
     long long ctas = (n_tasks + kWarps - 1) / kWarps;
-    if (ctas > 3LL * n_sms) ctas = 3LL * n_sms;   // persistent: 3 CTAs per SM pull from the queue
+    if (ctas > (long long)kCtasPerSm * n_sms) ctas = (long long)kCtasPerSm * n_sms;   // persistent CTAs pull from the queue
     const dim3 grid((unsigned)ctas), block(kWarps * 32);
     const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags, av = (uintptr_t)in.vis;
     const int opt = (in.weights ? kHasW : 0) | (in.flags ? kHasF : 0) | (d_density ? kHasD : 0);

@@ -2,6 +2,7 @@
 // the per-snapshot stage sequence a1..a7 and the streamed pipeline a8.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <chrono>
@@ -54,8 +55,8 @@ struct toi_plan {
     int snap_slot = 0;
     Inputs last_in = {nullptr, nullptr, nullptr, nullptr};
 
-    cufftHandle fft = 0;
-    bool fft_ok = false;
+    cufftHandle fft = 0, fft_cols = 0, fft_rows = 0;
+    bool fft_ok = false, fft_pruned = false;
     cudaStream_t s_compute = nullptr, s_copy = nullptr, fft_stream = nullptr;
     cudaEvent_t ev[EV_COUNT] = {};
     cudaEvent_t ev_h2d_start[2] = {}, ev_h2d_done[2] = {}, ev_c_start[2] = {}, ev_c_done[2] = {}, ev_first = nullptr;
@@ -139,6 +140,7 @@ int free_plan(toi_plan *p)
     if (p->s_compute) cudaStreamSynchronize(p->s_compute);
     if (p->s_copy) cudaStreamSynchronize(p->s_copy);
     if (p->fft_ok) cufftDestroy(p->fft);
+    if (p->fft_pruned) { cufftDestroy(p->fft_cols); cufftDestroy(p->fft_rows); }
     cudaFree(p->d_s); cudaFree(p->d_ipsi); cudaFree(p->d_V_inject); cudaFree(p->d_state);
     cudaFreeHost(p->h_state);
     for (int k = 0; k < 2; ++k) {
@@ -179,6 +181,9 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     int launches = 0;
     if (p->fft_stream != stream) {
         if (cufftSetStream(p->fft, stream) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
+        if (p->fft_pruned && (cufftSetStream(p->fft_cols, stream) != CUFFT_SUCCESS ||
+                              cufftSetStream(p->fft_rows, stream) != CUFFT_SUCCESS))
+            return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
         p->fft_stream = stream;
     }
     // buffers of this snapshot (zero-filled while the previous one was imaged) and, on s_zero, the
@@ -186,7 +191,16 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     const int k = (int)(p->ring_pos & 1), kn = k ^ 1;
     const bool uniform = p->cfg.weighting == TOI_WEIGHT_UNIFORM;
     float2 *const grid = p->d_grids[k];
+    // a1-a2: plane fit (also resets the per-snapshot accumulators)
+    launch_planefit(g, in.uvw, p->S1, p->S2, p->inject ? p->d_V_inject : nullptr, p->d_state, stream);
+    ++launches;
+    // this snapshot's buffers were zero-filled during the previous one; the cross-stream wait is
+    // placed after the plane fit (which touches neither) so that its latency hides under that kernel
     CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_zeroed[k], 0));
+    CU_TRY(p, cudaEventRecord(p->ev[EV_FIT], stream));
+    // zero fill of the other buffer pair for the next snapshot, on s_zero, once its last reader
+    // is done and after the plane fit (one latency-bound CTA that a saturating memset would slow)
+    CU_TRY(p, cudaStreamWaitEvent(p->s_zero, p->ev[EV_FIT], 0));
     CU_TRY(p, cudaStreamWaitEvent(p->s_zero, p->ev_free[kn], 0));
     CU_TRY(p, cudaEventRecord(p->ev_z0, p->s_zero));
     if (uniform) CU_TRY(p, cudaMemsetAsync(p->d_dens[kn], 0, GG * sizeof(float), p->s_zero));
@@ -194,10 +208,6 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     CU_TRY(p, cudaEventRecord(p->ev_z1, p->s_zero));
     CU_TRY(p, cudaEventRecord(p->ev_zeroed[kn], p->s_zero));
     launches += uniform ? 2 : 1;
-    // a1-a2: plane fit (also resets the per-snapshot accumulators)
-    launch_planefit(g, in.uvw, p->S1, p->S2, p->inject ? p->d_V_inject : nullptr, p->d_state, stream);
-    ++launches;
-    CU_TRY(p, cudaEventRecord(p->ev[EV_FIT], stream));
     // a4: uniform-weighting density pass
     const float *dens = nullptr;
     if (uniform) {
@@ -216,9 +226,21 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     if (p->keep_grid && p->d_grid_keep)
         CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
     // a6: inverse C2C FFT in place
-    if (cufftExecC2C(p->fft, (cufftComplex *)grid, (cufftComplex *)grid, CUFFT_INVERSE) != CUFFT_SUCCESS)
-        return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
-    ++launches;
+    if (p->fft_pruned) {
+        // row transforms of all G rows (contiguous), then column transforms of only the N columns
+        // the crop reads (columns n = -N/2..N/2-1 live at indices [0, N/2) and [G - N/2, G))
+        cufftComplex *F = (cufftComplex *)grid;
+        cufftComplex *Fhi = F + (g.G - g.N / 2);
+        if (cufftExecC2C(p->fft_rows, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
+            cufftExecC2C(p->fft_cols, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
+            cufftExecC2C(p->fft_cols, Fhi, Fhi, CUFFT_INVERSE) != CUFFT_SUCCESS)
+            return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
+        launches += 3;
+    } else {
+        if (cufftExecC2C(p->fft, (cufftComplex *)grid, (cufftComplex *)grid, CUFFT_INVERSE) != CUFFT_SUCCESS)
+            return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
+        ++launches;
+    }
     CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
     // a7: correction + crop + normalisation into the image ring
     float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
@@ -420,6 +442,23 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
         return TOI_ERR_CUFFT;
     }
     p->fft_ok = true;
+    // Pruned transform (default when the crop keeps at most 3/4 of the columns): 1-D transforms of
+    // all G rows, then of only the N columns the crop reads -- cuFFT's strided column pass is the
+    // expensive one (two kernels), so skipping G - N columns saves more than a third of the FFT.
+    // The skipped columns are left row-transformed only; nothing reads them.  TOI_FFT_PRUNED=0
+    // selects the plain 2-D plan.
+    bool pruned = 4 * N <= 3 * G;
+    if (const char *e = getenv("TOI_FFT_PRUNED")) pruned = pruned && atoi(e) != 0;
+    if (pruned) {
+        int n[1] = {G};
+        if (cufftPlanMany(&p->fft_cols, 1, n, n, G, 1, n, G, 1, CUFFT_C2C, N / 2) != CUFFT_SUCCESS ||
+            cufftPlanMany(&p->fft_rows, 1, n, n, 1, G, n, 1, G, CUFFT_C2C, G) != CUFFT_SUCCESS) {
+            fail(nullptr, TOI_ERR_CUFFT, "cufftPlanMany failed");
+            free_plan(p);
+            return TOI_ERR_CUFFT;
+        }
+        p->fft_pruned = true;
+    }
     CREATE_TRY(cudaDeviceSynchronize());
 #undef CREATE_TRY
     *out = p;
