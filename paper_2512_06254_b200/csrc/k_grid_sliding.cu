@@ -19,7 +19,7 @@
 //    reductions instead of 17 * 98 scalar atomics.
 //  * A warp carries four such groups (28 of 32 lanes) on four adjacent strips of one baseline.
 //    All 32 lanes first pre-process 32 samples (fp64 cell index, flags/weights/polarisation
-//    average, 14 kernel taps, packed for both axes, square root and exp2 on the MUFU pipe) into
+//    average, 14 kernel taps as even/odd polynomials packed for both axes) into
 //    an 80-byte shared-memory record each; the groups then consume their 8 records.  The consume
 //    phase is ONE inline-PTX block: the eight record bodies are straight-line code with
 //    immediate-offset LDS (next record's header prefetched), each with its own out-of-line

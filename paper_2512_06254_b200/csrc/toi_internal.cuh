@@ -158,31 +158,43 @@ __device__ __forceinline__ u64 mul2(u64 a, u64 b)
 }
 
 // Gridding kernel phi(x) = exp(beta_k (sqrt(1 - (2x/W)^2) - 1)) (G9) at the seven taps
-// du = -3..3 of a sample whose sub-cell offsets are (xu, xv) = g - i in [-0.5, 0.5]: tap distance
-// x = du - xoff, t = 2x/W.  Both axes are evaluated together as packed pairs:
-// 1 - t^2 = (1 - t)(1 + t) is two FFMA2 and one FMUL2, the exponent one FFMA2, and the square
-// root and exp2 go to the MUFU pipe.
+// k = -3..3 of a sample whose sub-cell offsets are (xu, xv) = g - i in [-0.5, 0.5]: tap distance
+// x = k - xoff.  phi is even, so phi(+-k - d) = E_k(d^2) +- d O_k(d^2) with one even and one odd
+// polynomial per PAIR of taps (degrees 4 and 3 in s = d^2; coefficients in tap_poly.inc, written by
+// gen_tap_poly.py from phi's definition; fit error <= 2.3e-8 absolute, below fp32 rounding of the
+// centre taps).  Both axes are evaluated together as packed pairs (FFMA2 with broadcast immediate
+// coefficients): 33 instructions for the 14 taps and nothing on the MUFU pipe, against 14 square
+// roots + 14 exp2 before.
+#include "tap_poly.inc"
+__device__ __forceinline__ u64 bcast2(float c) { return pack2(c, c); }
 __device__ __forceinline__ void kernel_taps2(float xu, float xv, float pu[kW], float pv[kW])
 {
-    constexpr float k2w = 2.0f / kW;
-    constexpr float kb2 = kBetaK * 1.4426950408889634f;   // beta_k * log2(e)
     const u64 X = pack2(xu, xv);
-#pragma unroll
-    for (int d = 0; d < kW; ++d) {
-        const float c = (float)(d - kH) * k2w;            // t = c - k2w * xoff
-        const u64 om = fma2(X, pack2(k2w, k2w), pack2(1.0f - c, 1.0f - c));     // 1 - t
-        const u64 op = fma2(X, pack2(-k2w, -k2w), pack2(1.0f + c, 1.0f + c));   // 1 + t
-        float2 a = unpack2(mul2(om, op));
-        // du = +3 reaches |x| = W/2 at xoff = -1/2 and du = -3 at xoff = +1/2 (an offset just below
-        // 1/2 rounds to 0.5f about once per 10^7 samples): rounding may leave 1 - t^2 at -1e-8
-        if (d == 0 || d == kW - 1) { a.x = fmaxf(a.x, 0.0f); a.y = fmaxf(a.y, 0.0f); }
-        float ru, rv;
-        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(ru) : "f"(a.x));
-        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(rv) : "f"(a.y));
-        const float2 e = unpack2(fma2(pack2(ru, rv), pack2(kb2, kb2), pack2(-kb2, -kb2)));
-        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(pu[d]) : "f"(e.x));
-        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(pv[d]) : "f"(e.y));
+    const u64 NX = pack2(-xu, -xv);
+    const u64 S = mul2(X, X);
+#define TOI_EVEN(k)                                                                               \
+    fma2(fma2(fma2(fma2(bcast2(TOI_TAP_E(k, 4)), S, bcast2(TOI_TAP_E(k, 3))), S, bcast2(TOI_TAP_E(k, 2))), S, \
+              bcast2(TOI_TAP_E(k, 1))), S, bcast2(TOI_TAP_E(k, 0)))
+#define TOI_ODD(k)                                                                                \
+    fma2(fma2(fma2(bcast2(TOI_TAP_O(k, 3)), S, bcast2(TOI_TAP_O(k, 2))), S, bcast2(TOI_TAP_O(k, 1))), S, \
+         bcast2(TOI_TAP_O(k, 0)))
+#define TOI_PAIR(k)                                                                               \
+    {                                                                                             \
+        const u64 E = TOI_EVEN(k), O = TOI_ODD(k);                                                \
+        const float2 hi = unpack2(fma2(X, O, E)), lo = unpack2(fma2(NX, O, E));                   \
+        pu[kH + k] = hi.x; pv[kH + k] = hi.y;                                                     \
+        pu[kH - k] = lo.x; pv[kH - k] = lo.y;                                                     \
     }
+    {
+        const float2 c = unpack2(TOI_EVEN(0));
+        pu[kH] = c.x; pv[kH] = c.y;
+    }
+    TOI_PAIR(1)
+    TOI_PAIR(2)
+    TOI_PAIR(3)
+#undef TOI_EVEN
+#undef TOI_ODD
+#undef TOI_PAIR
 }
 
 // ---- host-side launchers, one per translation unit -------------------------------------------

@@ -408,6 +408,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     CREATE_TRY(cudaMalloc(&p->d_state, sizeof(SnapState)));
     CREATE_TRY(cudaMemset(p->d_state, 0, sizeof(SnapState)));
     CREATE_TRY(cudaMallocHost(&p->h_state, sizeof(SnapState)));
+    // default (lowest) priority: measured, a high-priority fill slows the density pass by more than it hides
     CREATE_TRY(cudaStreamCreateWithFlags(&p->s_zero, cudaStreamNonBlocking));
     CREATE_TRY(cudaEventCreate(&p->ev_z0));
     CREATE_TRY(cudaEventCreate(&p->ev_z1));
