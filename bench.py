@@ -357,6 +357,20 @@ def run_e2e(r, args):
     return e2e, stream_res
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
+# `ncu --set full` captures summarised under profiles/ (a recorded measurement of the same command,
+# not something this run can observe).  The 134 MB grid zero fill is a separate cudaMemsetAsync and
+# most of the reductions stay in the 126 MB L2 until the FFT reads them, hence the small write figure.
+NCU_TRAFFIC = {
+    ("2", "uniform", "sliding"): {"bytes": 467278336 + 13732352, "source": "profiles/r1_k_grid_sliding_full.txt"},
+}
+
+
+def ncu_traffic(args, weighting):
+    t = NCU_TRAFFIC.get((str(args.workload), weighting, args.gridder))
+    return None if t is None else t["bytes"]
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -383,7 +397,7 @@ def main():
     achieved = ab["gridding"] / (grid_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "k_grid_%s (+ grid zero fill on the side stream)" % args.gridder, "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_8tbs_nominal": achieved / 8000.0,
-                "peak_source": peak_src, "traffic": None,
+                "peak_source": peak_src, "traffic": ncu_traffic(args, weighting),
                 "algorithmic_bytes": ab["gridding"], "ms": grid_ms, "ms_kernel": r["stages"]["ms_grid"],
                 "ms_zero_fill_alone": zero_alone_ms, "ms_zero_fill_in_situ": r["stages"]["ms_zero"], "ms_min": r["stages_min"]["ms_grid"],
                 "vis_per_s": r["S"] / (grid_ms * 1e-3)}
