@@ -155,6 +155,35 @@ typedef struct {
 int toi_image_stream(toi_plan *plan, int64_t n_snapshots, toi_fill_fn fill, void *fill_user,
                      toi_sink_fn sink, void *sink_user, int32_t want_info, toi_stream_stats *stats);
 
+/*
+ * Re-projection ("interpolate" stage, section 3.3 Eqs. 9-16, Appendix A): resample
+ * a dirty image from the tilted (t1, t2) plane it was reconstructed on to the standard (l, m) grid
+ * of the same size and cell size.  GATHER: output pixel (i, j) is the direction
+ * l = -beta (i - N/2), m = +beta (j - N/2); its place on the tilted image is (Eq. 16)
+ * p1' = N/2 - t1/beta, p2' = N/2 + t2/beta with
+ *   TOI_REPROJECT_EXACT  t = V s, s = (l, m, n - 1), n = sqrt(1 - l^2 - m^2)      (Eqs. 3-4)
+ *   TOI_REPROJECT_PAPER  t1 = l + xi z, t2 = m + eta z, z = 1 - n (Eq. 13),
+ *                        xi = V31/V33, eta = V32/V33 (Eqs. 14-15; sign reading DESIGN.md G16),
+ *                        the small-tilt reduction the paper evaluates
+ * and the value is the bilinear interpolation of the four neighbouring pixels (fp64 coordinates,
+ * fp32 values).  A position more than 1e-6 pixel outside [0, N-1]^2, or a direction outside the
+ * SIN domain (l^2 + m^2 > 1), gives NaN.  Readings G20-G23 of DESIGN.md.
+ *   d_image  DEVICE float32 [N][N], e.g. the pointer toi_image_snapshot returned
+ *   V        HOST row-major 3x3, or NULL = the transform of the snapshot most recently enqueued
+ *            by this plan (read on the device in stream order: enqueue on the same stream, before
+ *            the next snapshot).  With NULL a degenerate snapshot gives an all-NaN image.
+ *   d_out    DEVICE float32 [N][N], caller-owned, must not alias d_image
+ * Enqueues one kernel on cuda_stream (NULL = the plan's compute stream); does not synchronise.
+ */
+enum { TOI_REPROJECT_EXACT = 0, TOI_REPROJECT_PAPER = 1 };
+int toi_reproject(toi_plan *plan, const float *d_image, const double *V, int32_t mode, void *cuda_stream,
+                  float *d_out);
+
+/* Difference image d_out = d_a - d_b of two snapshots (what the downstream transient search
+ * consumes); DEVICE float32 [N][N] each, d_out may alias either input.  One kernel on
+ * cuda_stream (NULL = the plan's compute stream); does not synchronise. */
+int toi_difference(toi_plan *plan, const float *d_a, const float *d_b, void *cuda_stream, float *d_out);
+
 /* Human-readable description of the last error of this plan (or of plan creation when plan is
  * NULL); the string is owned by the library. */
 const char *toi_last_error(const toi_plan *plan);

@@ -15,7 +15,9 @@ Readings (G20-G23; the paper leaves all four open):
        "paper" evaluates Eqs. 9-16 literally (tilt enters only through xi = V31/V33, eta = V32/V33).
   G16  Eq. 11/15 sign garble: y' = y + r0 z eta (Appendix A6 has the outer minus), x' = x + r0 z xi.
   G22  interpolation: bilinear on the four neighbours (the paper names none); a pixel whose source
-       position falls outside [0, N-1]^2, or outside the SIN domain h <= r0, is NaN.
+       position falls outside [0, N-1]^2, or outside the SIN domain h <= r0, is NaN.  A position
+       within 1e-6 px outside the edge is taken as on the edge (with V = I the positions are the
+       integers up to rounding, and the last row/column must not depend on that rounding).
   G23  pixel convention as everywhere else (G6): 0-based, centre N/2, x = -beta (i - N/2),
        y = +beta (j - N/2); Eq. 9's 1-based (N/2 + 1) is the same pixel.
 
@@ -128,13 +130,14 @@ def map_exact(V, N, cell_size_deg):
 
 def bilinear_gather(image, p1, p2, valid):
     """G22: out[j][i] = bilinear(image at column p1[j][i], row p2[j][i]); NaN where the position is
-    invalid or outside [0, N-1]^2.  Plain definition, no vector tricks beyond numpy indexing."""
+    invalid or outside [0, N-1]^2 (by more than 1e-6 px).  Plain definition, no vector tricks beyond numpy indexing."""
     img = np.asarray(image, dtype=np.float64)
     N = img.shape[0]
     assert img.shape == (N, N)
-    inside = valid & (p1 >= 0.0) & (p1 <= N - 1.0) & (p2 >= 0.0) & (p2 <= N - 1.0)
-    a = np.where(inside, p1, 0.0)
-    b = np.where(inside, p2, 0.0)
+    eps = 1e-6          # G22: a position within 1e-6 px outside the edge counts as on the edge
+    inside = valid & (p1 >= -eps) & (p1 <= N - 1.0 + eps) & (p2 >= -eps) & (p2 <= N - 1.0 + eps)
+    a = np.clip(np.where(inside, p1, 0.0), 0.0, N - 1.0)
+    b = np.clip(np.where(inside, p2, 0.0), 0.0, N - 1.0)
     i0 = np.minimum(np.floor(a), N - 2).astype(np.int64)
     j0 = np.minimum(np.floor(b), N - 2).astype(np.int64)
     fx = a - i0

@@ -19,9 +19,11 @@ TOI_ERR_DEGENERATE_GEOMETRY, TOI_ERR_CALLBACK, TOI_ERR_UNSUPPORTED = -5, -6, -7
 TOI_WEIGHT_NATURAL, TOI_WEIGHT_UNIFORM = 0, 1
 TOI_MEM_HOST, TOI_MEM_DEVICE = 0, 1
 TOI_GRIDDER_SLIDING, TOI_GRIDDER_ATOMIC = 0, 1
+TOI_REPROJECT_EXACT, TOI_REPROJECT_PAPER = 0, 1
 
 EXPORTS = ["toi_plan_create", "toi_plan_destroy", "toi_image_snapshot", "toi_plan_sync",
-           "toi_copy_image_to_host", "toi_image_stream", "toi_last_error", "toi_last_launch_count",
+           "toi_copy_image_to_host", "toi_image_stream", "toi_reproject", "toi_difference",
+           "toi_last_error", "toi_last_launch_count",
            "toi_debug_set_transform", "toi_debug_cell_indices", "toi_debug_keep_grid",
            "toi_debug_copy_grid", "toi_debug_copy_density"]
 
@@ -94,6 +96,8 @@ def load(build_if_missing: bool = True):
     lib.toi_plan_sync.argtypes = [vp]
     lib.toi_copy_image_to_host.argtypes = [vp, vp, vp]
     lib.toi_image_stream.argtypes = [vp, i64, toi_fill_fn, vp, toi_sink_fn, vp, i32, C.POINTER(toi_stream_stats)]
+    lib.toi_reproject.argtypes = [vp, vp, vp, i32, vp, vp]
+    lib.toi_difference.argtypes = [vp, vp, vp, vp, vp]
     lib.toi_last_error.argtypes = [vp]
     lib.toi_last_error.restype = C.c_char_p
     lib.toi_last_launch_count.argtypes = [vp]
@@ -199,6 +203,30 @@ def toi_image_stream(plan, n_snapshots, fill, sink=None, want_info=False):
     rc = lib.toi_image_stream(plan, int(n_snapshots), cfill, None, csink, None, 1 if want_info else 0, C.byref(stats))
     _check(plan, rc)
     return stats.as_dict()
+
+
+def _dev(x):
+    """A device address: a CUDA tensor or the int toi_image_snapshot returned."""
+    return C.c_void_p(x) if isinstance(x, int) else _ptr(x)
+
+
+def toi_reproject(plan, d_image, out, V=None, mode=TOI_REPROJECT_EXACT, stream=None):
+    """d_image: device pointer (int) or CUDA tensor [N, N] f32 on the tilted plane; out: CUDA tensor
+    [N, N] f32 (written); V: 3x3 (host) or None = the plan's last snapshot.  Enqueues only."""
+    v = None
+    if V is not None:
+        v = torch.as_tensor(V, dtype=torch.float64, device="cpu").contiguous().reshape(9)
+    s = None if stream is None else C.c_void_p(stream.cuda_stream)
+    _check(plan, load().toi_reproject(plan, _dev(d_image), None if v is None else C.c_void_p(v.data_ptr()),
+                                      int(mode), s, _dev(out)))
+    return out
+
+
+def toi_difference(plan, d_a, d_b, out, stream=None):
+    """out = a - b, device [N, N] f32 each (pointers or CUDA tensors).  Enqueues only."""
+    s = None if stream is None else C.c_void_p(stream.cuda_stream)
+    _check(plan, load().toi_difference(plan, _dev(d_a), _dev(d_b), s, _dev(out)))
+    return out
 
 
 def toi_last_error(plan=None):

@@ -207,6 +207,9 @@ void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, con
                          float2 *d_grid, int n_sms, cudaStream_t stream);
 void launch_correct_crop(const Geometry &g, const float2 *d_F, const double *d_ipsi, const SnapState *st,
                          int apply_jacobian, float *d_image, cudaStream_t stream);
+void launch_reproject(int N, double beta_rad, const SnapState *st, const double *d_V, int mode, const float *d_src,
+                      float *d_dst, cudaStream_t stream);
+void launch_difference(size_t n, const float *d_a, const float *d_b, float *d_out, int n_sms, cudaStream_t stream);
 void launch_cell_indices(const Geometry &g, const double *d_uvw, const SnapState *st, int32_t *d_iu,
                          int32_t *d_iv, cudaStream_t stream);
 

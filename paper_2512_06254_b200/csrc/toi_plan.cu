@@ -36,7 +36,7 @@ struct toi_plan {
     int apply_jacobian = 1;
     size_t n_samples = 0, n_elems = 0;
 
-    double *d_s = nullptr, *d_ipsi = nullptr, *d_V_inject = nullptr;
+    double *d_s = nullptr, *d_ipsi = nullptr, *d_V_inject = nullptr, *d_V_reproject = nullptr;
     SnapState *d_state = nullptr, *h_state = nullptr;
     DevSlot dev_in[2];
     toi_snapshot_buffers pin[2] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
@@ -141,7 +141,7 @@ int free_plan(toi_plan *p)
     if (p->s_copy) cudaStreamSynchronize(p->s_copy);
     if (p->fft_ok) cufftDestroy(p->fft);
     if (p->fft_pruned) { cufftDestroy(p->fft_cols); cufftDestroy(p->fft_rows); }
-    cudaFree(p->d_s); cudaFree(p->d_ipsi); cudaFree(p->d_V_inject); cudaFree(p->d_state);
+    cudaFree(p->d_s); cudaFree(p->d_ipsi); cudaFree(p->d_V_inject); cudaFree(p->d_V_reproject); cudaFree(p->d_state);
     cudaFreeHost(p->h_state);
     for (int k = 0; k < 2; ++k) {
         cudaFree(p->dev_in[k].uvw); cudaFree(p->dev_in[k].vis);
@@ -405,6 +405,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     CREATE_TRY(cudaMalloc(&p->d_ipsi, (size_t)N * sizeof(double)));
     CREATE_TRY(cudaMemcpy(p->d_ipsi, ipsi.data(), (size_t)N * sizeof(double), cudaMemcpyHostToDevice));
     CREATE_TRY(cudaMalloc(&p->d_V_inject, 9 * sizeof(double)));
+    CREATE_TRY(cudaMalloc(&p->d_V_reproject, 9 * sizeof(double)));
     CREATE_TRY(cudaMalloc(&p->d_state, sizeof(SnapState)));
     CREATE_TRY(cudaMemset(p->d_state, 0, sizeof(SnapState)));
     CREATE_TRY(cudaMallocHost(&p->h_state, sizeof(SnapState)));
@@ -593,6 +594,36 @@ int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *f
         if (p->deferred != TOI_OK) { rc = p->deferred; p->deferred = TOI_OK; }
     }
     return rc;
+}
+
+int toi_reproject(toi_plan *p, const float *d_image, const double *V, int32_t mode, void *cuda_stream, float *d_out)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    if (!d_image || !d_out || d_image == d_out) return fail(p, TOI_ERR_INVALID_ARG, "d_image and d_out must be non-NULL and distinct");
+    if (mode != TOI_REPROJECT_EXACT && mode != TOI_REPROJECT_PAPER) return fail(p, TOI_ERR_INVALID_ARG, "unknown re-projection mode");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    cudaStream_t stream = cuda_stream ? (cudaStream_t)cuda_stream : p->s_compute;
+    if (V) {
+        for (int k = 0; k < 9; ++k)
+            if (!isfinite(V[k])) return fail(p, TOI_ERR_INVALID_ARG, "V must be finite");
+        if (!(fabs(V[8]) >= 1e-6)) return fail(p, TOI_ERR_DEGENERATE_GEOMETRY, "V33 < 1e-6: no tilted plane to re-project from");
+        CU_TRY(p, cudaMemcpyAsync(p->d_V_reproject, V, 9 * sizeof(double), cudaMemcpyHostToDevice, stream));
+    }
+    const double beta_rad = p->cfg.cell_size_deg * (3.14159265358979323846 / 180.0);
+    launch_reproject(p->geo.N, beta_rad, p->d_state, V ? p->d_V_reproject : nullptr, mode, d_image, d_out, stream);
+    CU_TRY(p, cudaGetLastError());
+    return TOI_OK;
+}
+
+int toi_difference(toi_plan *p, const float *d_a, const float *d_b, void *cuda_stream, float *d_out)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    if (!d_a || !d_b || !d_out) return fail(p, TOI_ERR_INVALID_ARG, "NULL argument");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    cudaStream_t stream = cuda_stream ? (cudaStream_t)cuda_stream : p->s_compute;
+    launch_difference((size_t)p->geo.N * p->geo.N, d_a, d_b, d_out, p->n_sms, stream);
+    CU_TRY(p, cudaGetLastError());
+    return TOI_OK;
 }
 
 const char *toi_last_error(const toi_plan *plan) { return plan ? plan->err : g_create_error; }
