@@ -261,6 +261,28 @@ def run_ours(args):
     stages = {k: sum(v) / len(v) for k, v in acc.items()}
     stages_min = {k: min(v) for k, v in acc.items()}
     n_gridded = int(info.n_gridded)
+    # ---------------- NEXT rows, timed on their own (not part of `value`): re-projection of the
+    # image just made with the snapshot's own V, and the difference of two ring images ----------------
+    ptr_a, _, _ = toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
+    ptr_b, _, _ = toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
+    out_img = torch.empty((N, N), dtype=torch.float32, device="cuda")
+    extra = {}
+    for name, fn in (("ms_reproject", lambda: toi.toi_reproject(plan, ptr_b, out_img, stream=stream)),
+                     ("ms_difference", lambda: toi.toi_difference(plan, ptr_b, ptr_a, out_img, stream=stream))):
+        for _ in range(3):
+            fn()
+        best, tot, reps = 1e9, 0.0, 10
+        for _ in range(reps):
+            x0, x1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            x0.record(stream)
+            fn()
+            x1.record(stream)
+            torch.cuda.synchronize()
+            t = x0.elapsed_time(x1)
+            best, tot = min(best, t), tot + t
+        extra[name] = tot / reps
+        extra[name + "_min"] = best
+    del out_img
     toi.toi_plan_destroy(plan)
     # the grid's zero fill alone (same size, same API call the library uses), best of 5
     zbuf = torch.empty(4 * N * N * 2, dtype=torch.float32, device="cuda")   # G x G complex64
@@ -277,7 +299,7 @@ def run_ours(args):
     return dict(rank=rank, local=local, world=world, wl=wl, weighting=weighting, wt=wt, gridder=gridder, S=S, N=N,
                 snap=snap, freq=freq, stream=stream, ms_step=ms_step, value=value, clocks=clocks, stages=stages,
                 stages_min=stages_min, n_gridded=n_gridded, launches_per_step=launches_per_step,
-                zero_alone_ms=zero_alone_ms)
+                zero_alone_ms=zero_alone_ms, extra=extra)
 
 
 def pinned_h2d_peak_gbs(n_bytes=1 << 30, repeats=5):
@@ -353,6 +375,23 @@ def run_e2e(r, args):
                       "h2d_ms_mean": st["h2d_ms_sum"] / max(1, st["n_done"]),
                       "compute_ms_mean": st["compute_ms_sum"] / max(1, st["n_done"]),
                       "source": "replay pool of 1 pinned snapshot (DESIGN.md section 4); images stay on the GPU"}
+        # the same stream with the output side on: re-projection of every image (interpolate stage)
+        # and its D2H through the pinned ring to a host sink (copy_cpu stage)
+        seen = []
+        toi.toi_stream_set_output(plan, product=toi.TOI_OUT_REPROJECT_EXACT,
+                                  host_sink=lambda idx, image: seen.append(idx), image_size=N)
+        toi.toi_image_stream(plan, 4, fill)
+        del seen[:]
+        st = toi.toi_image_stream(plan, args.stream_snapshots, fill)
+        stream_res["with_output"] = {
+            "snapshots": int(st["n_done"]), "images_on_host": len(seen),
+            "ms_per_snapshot": st["gpu_ms"] / max(1, st["n_done"]),
+            "wall_ms_per_snapshot": 1e3 * st["wall_s"] / max(1, st["n_done"]),
+            "h2d_gbs": st["h2d_bytes"] / (st["gpu_ms"] * 1e-3) / 1e9,
+            "d2h_bytes_per_snapshot": st["d2h_bytes"] / max(1, st["n_done"]),
+            "d2h_ms_mean": st["d2h_ms_sum"] / max(1, st["n_done"]),
+            "what": "re-projected (exact) image of every snapshot delivered to a host callback"}
+        toi.toi_stream_set_output(plan)
     toi.toi_plan_destroy(plan)
     return e2e, stream_res
 
@@ -406,6 +445,12 @@ def main():
         stages["density_gbs"] = ab["density"] / ((r["stages"]["ms_weight"] + 0.5 * zero_alone_ms) * 1e-3) / 1e9
     stages["fft_gbs_min_traffic"] = ab["fft_min"] / (r["stages"]["ms_fft"] * 1e-3) / 1e9
     stages["crop_gbs"] = ab["crop"] / (r["stages"]["ms_crop"] * 1e-3) / 1e9
+    # NEXT rows, timed alone: N^2 x (4 read + 4 written) resp. (8 read + 4 written)
+    n2 = float(r["N"]) ** 2
+    stages["ms_reproject"] = round(r["extra"]["ms_reproject"], 5)
+    stages["reproject_gbs"] = n2 * 8 / (r["extra"]["ms_reproject_min"] * 1e-3) / 1e9
+    stages["ms_difference"] = round(r["extra"]["ms_difference"], 5)
+    stages["difference_gbs"] = n2 * 12 / (r["extra"]["ms_difference_min"] * 1e-3) / 1e9
     pcie = pinned_h2d_peak_gbs()
     e2e["pcie_peak_gbs_measured"] = pcie
     e2e["pcie_frac"] = e2e["h2d_gbs_per_gpu"] / pcie

@@ -150,7 +150,39 @@ typedef struct {
     double h2d_bytes;           /* total bytes copied host -> device */
     double h2d_ms_sum;          /* sum of per-snapshot H2D durations (events) */
     double compute_ms_sum;      /* sum of per-snapshot imaging durations (events) */
+    double d2h_bytes;           /* total bytes copied device -> host (toi_stream_set_output.to_host) */
+    double d2h_ms_sum;          /* sum of per-image D2H durations (events) */
 } toi_stream_stats;
+
+/*
+ * Output side of the streamed run (the paper's `interpolate` and `copy_cpu` stages, PAPER.md:302-304,
+ * 345, 355): what toi_image_stream delivers for every snapshot.
+ *   product     TOI_OUT_TILTED: the dirty image on the tilted plane (default);
+ *               TOI_OUT_REPROJECT_EXACT / _PAPER: that image re-projected to the (l, m) grid (see
+ *               toi_reproject) with the snapshot's own V, into a second device ring of the plan's
+ *               image_ring_depth (the interpolate stage owns the image ring)
+ *   difference  1: deliver product(n) - product(n-1) instead; snapshot 0 has no
+ *               predecessor and delivers its product to the device sink and nothing to the host sink
+ *   to_host     1: copy every delivered image device -> host on a third stream through a depth-2
+ *               PINNED ring (cudaMemcpyAsync only, events between the streams) and
+ *               call host_sink(user, idx, h_image) once it has landed -- in index order, from the
+ *               thread running toi_image_stream, up to two snapshots after idx was enqueued (all
+ *               before toi_image_stream returns).  h_image is valid until the callback returns.
+ *               Needs image_ring_depth >= 2.  A negative return aborts the run (TOI_ERR_CALLBACK).
+ * The device sink of toi_image_stream receives the delivered image (difference or product).
+ * Everything this needs is allocated HERE, not in the loop.  NULL restores the default.
+ */
+enum { TOI_OUT_TILTED = 0, TOI_OUT_REPROJECT_EXACT = 1, TOI_OUT_REPROJECT_PAPER = 2 };
+typedef int (*toi_host_sink_fn)(void *user, int64_t idx, const float *h_image);
+typedef struct {
+    int32_t product;
+    int32_t difference;
+    int32_t to_host;
+    int32_t reserved[5];        /* must be 0 */
+    toi_host_sink_fn host_sink; /* required when to_host */
+    void *host_user;
+} toi_stream_output;
+int toi_stream_set_output(toi_plan *plan, const toi_stream_output *out);
 
 int toi_image_stream(toi_plan *plan, int64_t n_snapshots, toi_fill_fn fill, void *fill_user,
                      toi_sink_fn sink, void *sink_user, int32_t want_info, toi_stream_stats *stats);

@@ -20,9 +20,10 @@ TOI_WEIGHT_NATURAL, TOI_WEIGHT_UNIFORM = 0, 1
 TOI_MEM_HOST, TOI_MEM_DEVICE = 0, 1
 TOI_GRIDDER_SLIDING, TOI_GRIDDER_ATOMIC = 0, 1
 TOI_REPROJECT_EXACT, TOI_REPROJECT_PAPER = 0, 1
+TOI_OUT_TILTED, TOI_OUT_REPROJECT_EXACT, TOI_OUT_REPROJECT_PAPER = 0, 1, 2
 
 EXPORTS = ["toi_plan_create", "toi_plan_destroy", "toi_image_snapshot", "toi_plan_sync",
-           "toi_copy_image_to_host", "toi_image_stream", "toi_reproject", "toi_difference",
+           "toi_copy_image_to_host", "toi_image_stream", "toi_stream_set_output", "toi_reproject", "toi_difference",
            "toi_last_error", "toi_last_launch_count",
            "toi_debug_set_transform", "toi_debug_cell_indices", "toi_debug_keep_grid",
            "toi_debug_copy_grid", "toi_debug_copy_density"]
@@ -57,7 +58,8 @@ class toi_snapshot_buffers(C.Structure):
 
 class toi_stream_stats(C.Structure):
     _fields_ = [("n_done", C.c_int64), ("wall_s", C.c_double), ("gpu_ms", C.c_double),
-                ("h2d_bytes", C.c_double), ("h2d_ms_sum", C.c_double), ("compute_ms_sum", C.c_double)]
+                ("h2d_bytes", C.c_double), ("h2d_ms_sum", C.c_double), ("compute_ms_sum", C.c_double),
+                ("d2h_bytes", C.c_double), ("d2h_ms_sum", C.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -65,6 +67,15 @@ class toi_stream_stats(C.Structure):
 
 toi_fill_fn = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int64, C.POINTER(toi_snapshot_buffers))
 toi_sink_fn = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(toi_snapshot_info))
+toi_host_sink_fn = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int64, C.c_void_p)
+
+
+class toi_stream_output(C.Structure):
+    _fields_ = [("product", C.c_int32), ("difference", C.c_int32), ("to_host", C.c_int32),
+                ("reserved", C.c_int32 * 5), ("host_sink", toi_host_sink_fn), ("host_user", C.c_void_p)]
+
+
+_host_sinks = {}      # plan address -> ctypes callback kept alive while the plan may call it
 
 _lib = None
 
@@ -96,6 +107,7 @@ def load(build_if_missing: bool = True):
     lib.toi_plan_sync.argtypes = [vp]
     lib.toi_copy_image_to_host.argtypes = [vp, vp, vp]
     lib.toi_image_stream.argtypes = [vp, i64, toi_fill_fn, vp, toi_sink_fn, vp, i32, C.POINTER(toi_stream_stats)]
+    lib.toi_stream_set_output.argtypes = [vp, C.POINTER(toi_stream_output)]
     lib.toi_reproject.argtypes = [vp, vp, vp, i32, vp, vp]
     lib.toi_difference.argtypes = [vp, vp, vp, vp, vp]
     lib.toi_last_error.argtypes = [vp]
@@ -147,6 +159,7 @@ def toi_plan_create(n_baselines, n_channels, n_pols, chan_freq_hz, image_size, c
 
 
 def toi_plan_destroy(plan):
+    _host_sinks.pop(getattr(plan, "value", None), None)
     return load().toi_plan_destroy(plan)
 
 
@@ -203,6 +216,35 @@ def toi_image_stream(plan, n_snapshots, fill, sink=None, want_info=False):
     rc = lib.toi_image_stream(plan, int(n_snapshots), cfill, None, csink, None, 1 if want_info else 0, C.byref(stats))
     _check(plan, rc)
     return stats.as_dict()
+
+
+def toi_stream_set_output(plan, product=TOI_OUT_TILTED, difference=False, host_sink=None, image_size=None):
+    """Output side of toi_image_stream.  host_sink(idx, image: float32 numpy view [N, N] of the pinned
+    slot, valid during the call) -> None/int enables the D2H ring; product/difference as in toi.h.
+    Call with no arguments to restore the default."""
+    import numpy as np
+    cb = C.cast(None, toi_host_sink_fn)
+    if host_sink is not None:
+        assert image_size, "image_size is needed to view the host image"
+        n = int(image_size)
+
+        def _hs(user, idx, h_image):
+            try:
+                buf = (C.c_float * (n * n)).from_address(h_image)
+                r = host_sink(idx, np.frombuffer(buf, dtype=np.float32).reshape(n, n))
+                return 0 if r is None else int(r)
+            except Exception:      # never unwind through C
+                import traceback
+                traceback.print_exc()
+                return -1
+
+        cb = toi_host_sink_fn(_hs)
+    o = toi_stream_output(int(product), 1 if difference else 0, 0 if host_sink is None else 1)
+    o.host_sink = cb
+    rc = load().toi_stream_set_output(plan, C.byref(o))
+    _check(plan, rc)
+    _host_sinks[plan.value] = cb
+    return rc
 
 
 def _dev(x):

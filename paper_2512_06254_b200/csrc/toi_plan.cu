@@ -61,6 +61,13 @@ struct toi_plan {
     cudaEvent_t ev[EV_COUNT] = {};
     cudaEvent_t ev_h2d_start[2] = {}, ev_h2d_done[2] = {}, ev_c_start[2] = {}, ev_c_done[2] = {}, ev_first = nullptr;
 
+    // output side of the streamed run (toi_stream_set_output): re-projected image ring, difference
+    // ping-pong, pinned depth-2 D2H ring on its own stream
+    toi_stream_output out_cfg = {};
+    float *d_products = nullptr, *d_diff[2] = {nullptr, nullptr}, *h_out[2] = {nullptr, nullptr};
+    cudaStream_t s_d2h = nullptr;
+    cudaEvent_t ev_out_ready[2] = {}, ev_d2h_start[2] = {}, ev_d2h_done[2] = {}, ev_tail = nullptr;
+
     int deferred = TOI_OK;
     int last_launches = 0;
     char err[512] = "";
@@ -165,6 +172,17 @@ int free_plan(toi_plan *p)
     if (p->ev_z0) cudaEventDestroy(p->ev_z0);
     if (p->ev_z1) cudaEventDestroy(p->ev_z1);
     if (p->s_zero) cudaStreamDestroy(p->s_zero);
+    if (p->s_d2h) cudaStreamSynchronize(p->s_d2h);
+    cudaFree(p->d_products);
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(p->d_diff[k]);
+        cudaFreeHost(p->h_out[k]);
+        if (p->ev_out_ready[k]) cudaEventDestroy(p->ev_out_ready[k]);
+        if (p->ev_d2h_start[k]) cudaEventDestroy(p->ev_d2h_start[k]);
+        if (p->ev_d2h_done[k]) cudaEventDestroy(p->ev_d2h_done[k]);
+    }
+    if (p->ev_tail) cudaEventDestroy(p->ev_tail);
+    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
     cudaFree(p->d_grid_keep); cudaFree(p->d_images);
     if (p->s_compute) cudaStreamDestroy(p->s_compute);
     if (p->s_copy) cudaStreamDestroy(p->s_copy);
@@ -517,6 +535,42 @@ int toi_copy_image_to_host(toi_plan *p, const float *d_image, float *h_image)
     return TOI_OK;
 }
 
+int toi_stream_set_output(toi_plan *p, const toi_stream_output *out)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    toi_stream_output o;
+    memset(&o, 0, sizeof o);
+    if (out) o = *out;
+    if (o.product != TOI_OUT_TILTED && o.product != TOI_OUT_REPROJECT_EXACT && o.product != TOI_OUT_REPROJECT_PAPER)
+        return fail(p, TOI_ERR_INVALID_ARG, "unknown stream product");
+    if ((o.difference != 0 && o.difference != 1) || (o.to_host != 0 && o.to_host != 1))
+        return fail(p, TOI_ERR_INVALID_ARG, "difference and to_host must be 0 or 1");
+    for (int k = 0; k < 5; ++k)
+        if (o.reserved[k] != 0) return fail(p, TOI_ERR_INVALID_ARG, "reserved fields must be 0");
+    if (o.to_host && !o.host_sink) return fail(p, TOI_ERR_INVALID_ARG, "to_host needs a host_sink callback");
+    if ((o.to_host || o.difference) && p->ring_depth < 2)
+        return fail(p, TOI_ERR_INVALID_ARG, "difference / to_host need image_ring_depth >= 2");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    CU_TRY(p, cudaDeviceSynchronize());
+    const size_t img_bytes = (size_t)p->geo.N * p->geo.N * sizeof(float);
+    if (!p->ev_tail) CU_TRY(p, cudaEventCreate(&p->ev_tail));
+    if (o.product != TOI_OUT_TILTED && !p->d_products) CU_TRY(p, cudaMalloc(&p->d_products, (size_t)p->ring_depth * img_bytes));
+    if (o.difference)
+        for (int k = 0; k < 2; ++k)
+            if (!p->d_diff[k]) CU_TRY(p, cudaMalloc(&p->d_diff[k], img_bytes));
+    if (o.to_host) {
+        if (!p->s_d2h) CU_TRY(p, cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
+        for (int k = 0; k < 2; ++k) {
+            if (!p->h_out[k]) CU_TRY(p, cudaMallocHost(&p->h_out[k], img_bytes));
+            if (!p->ev_out_ready[k]) CU_TRY(p, cudaEventCreateWithFlags(&p->ev_out_ready[k], cudaEventDisableTiming));
+            if (!p->ev_d2h_start[k]) CU_TRY(p, cudaEventCreate(&p->ev_d2h_start[k]));
+            if (!p->ev_d2h_done[k]) CU_TRY(p, cudaEventCreate(&p->ev_d2h_done[k]));
+        }
+    }
+    p->out_cfg = o;
+    return TOI_OK;
+}
+
 int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *fill_user, toi_sink_fn sink,
                      void *sink_user, int32_t want_info, toi_stream_stats *stats)
 {
@@ -535,6 +589,22 @@ int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *f
         if (cudaEventSynchronize(p->ev_c_done[slot]) != cudaSuccess) return;
         if (cudaEventElapsedTime(&ms, p->ev_h2d_start[slot], p->ev_h2d_done[slot]) == cudaSuccess) st.h2d_ms_sum += ms;
         if (cudaEventElapsedTime(&ms, p->ev_c_start[slot], p->ev_c_done[slot]) == cudaSuccess) st.compute_ms_sum += ms;
+    };
+    // ---- output side (toi_stream_set_output) ----
+    const toi_stream_output oc = p->out_cfg;
+    const size_t n_pix = (size_t)p->geo.N * p->geo.N;
+    const double beta_rad = p->cfg.cell_size_deg * (3.14159265358979323846 / 180.0);
+    const float *prev_prod = nullptr;
+    int64_t out_idx[2] = {-1, -1}, n_out = 0;
+    bool tail_used = false;
+    auto finish_out = [&](int o, bool call) -> int {   // the D2H in pinned slot o has landed: hand it over
+        if (out_idx[o] < 0) return TOI_OK;
+        const int64_t idx = out_idx[o];
+        out_idx[o] = -1;
+        if (cudaEventSynchronize(p->ev_d2h_done[o]) != cudaSuccess) return fail(p, TOI_ERR_CUDA, "D2H of an output image failed");
+        if (cudaEventElapsedTime(&ms, p->ev_d2h_start[o], p->ev_d2h_done[o]) == cudaSuccess) st.d2h_ms_sum += ms;
+        if (call && oc.host_sink(oc.host_user, idx, p->h_out[o]) < 0) return fail(p, TOI_ERR_CALLBACK, "host sink callback failed");
+        return TOI_OK;
     };
     int64_t n = 0;
     for (; n < n_snapshots; ++n) {
@@ -567,24 +637,80 @@ int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *f
         if (rc) break;
         CU_TRY(p, cudaEventRecord(p->ev_c_done[slot], p->s_compute));
         used[slot] = true;
+        // interpolate stage: tilted plane -> (l, m) grid with this snapshot's V
+        float *prod = img;
+        if (oc.product != TOI_OUT_TILTED) {
+            prod = p->d_products + (size_t)((p->ring_pos - 1) % p->ring_depth) * n_pix;
+            launch_reproject(p->geo.N, beta_rad, p->d_state, nullptr,
+                             oc.product == TOI_OUT_REPROJECT_PAPER ? TOI_REPROJECT_PAPER : TOI_REPROJECT_EXACT, img, prod,
+                             p->s_compute);
+        }
+        const float *deliver = prod;
+        bool to_host = oc.to_host != 0;
+        const int o = (int)(n_out & 1);
+        if (to_host && (!oc.difference || prev_prod)) {
+            // pinned slot o (and the difference buffer it was copied from) is free once the D2H
+            // two deliveries ago has landed; its image goes to the host sink now
+            rc = finish_out(o, true);
+            if (rc) break;
+        }
+        if (oc.difference) {
+            if (prev_prod) {
+                launch_difference(n_pix, prod, prev_prod, p->d_diff[n & 1], p->n_sms, p->s_compute);
+                deliver = p->d_diff[n & 1];
+            } else {
+                to_host = false;                  // snapshot 0 has no predecessor
+            }
+            prev_prod = prod;
+        }
+        if (oc.product != TOI_OUT_TILTED || oc.difference) {
+            CU_TRY(p, cudaGetLastError());
+            CU_TRY(p, cudaEventRecord(p->ev_tail, p->s_compute));
+            tail_used = true;
+        }
+        if (to_host) {
+            // copy_cpu stage: third stream, pinned ring, events only
+            CU_TRY(p, cudaEventRecord(p->ev_out_ready[o], p->s_compute));
+            CU_TRY(p, cudaStreamWaitEvent(p->s_d2h, p->ev_out_ready[o], 0));
+            CU_TRY(p, cudaEventRecord(p->ev_d2h_start[o], p->s_d2h));
+            CU_TRY(p, cudaMemcpyAsync(p->h_out[o], deliver, n_pix * sizeof(float), cudaMemcpyDeviceToHost, p->s_d2h));
+            CU_TRY(p, cudaEventRecord(p->ev_d2h_done[o], p->s_d2h));
+            out_idx[o] = n;
+            ++n_out;
+            st.d2h_bytes += (double)(n_pix * sizeof(float));
+        }
         toi_snapshot_info info;
         if (want_info) {
             rc = read_info(p, p->s_compute, &info, false);
             if (rc) break;
         }
         if (sink) {
-            const int src = sink(sink_user, n, img, (void *)p->s_compute, want_info ? &info : nullptr);
+            const int src = sink(sink_user, n, deliver, (void *)p->s_compute, want_info ? &info : nullptr);
             if (src < 0) { rc = fail(p, TOI_ERR_CALLBACK, "sink callback failed"); break; }
         }
     }
     cudaStreamSynchronize(p->s_copy);
     cudaStreamSynchronize(p->s_compute);
+    if (p->s_d2h) cudaStreamSynchronize(p->s_d2h);
+    {   // drain the host ring in index order
+        const int first = (out_idx[0] >= 0 && (out_idx[1] < 0 || out_idx[0] < out_idx[1])) ? 0 : 1;
+        float tail_ms = 0.0f;
+        for (int k = 0; k < 2; ++k) {
+            const int oo = k == 0 ? first : first ^ 1;
+            if (out_idx[oo] < 0) continue;
+            if (cudaEventElapsedTime(&ms, p->ev_first, p->ev_d2h_done[oo]) == cudaSuccess && ms > tail_ms) tail_ms = ms;
+            const int frc = finish_out(oo, rc == TOI_OK);
+            if (rc == TOI_OK) rc = frc;
+        }
+        if (tail_used && cudaEventElapsedTime(&ms, p->ev_first, p->ev_tail) == cudaSuccess && ms > tail_ms) tail_ms = ms;
+        st.gpu_ms = tail_ms;
+    }
     st.n_done = n;
     for (int slot = 0; slot < 2; ++slot)
         if (used[slot]) harvest(slot);
     if (n > 0) {
         const int last = (int)((n - 1) & 1);
-        if (cudaEventElapsedTime(&ms, p->ev_first, p->ev_c_done[last]) == cudaSuccess) st.gpu_ms = ms;
+        if (cudaEventElapsedTime(&ms, p->ev_first, p->ev_c_done[last]) == cudaSuccess && ms > st.gpu_ms) st.gpu_ms = ms;
     }
     cudaGetLastError();
     st.wall_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();

@@ -193,3 +193,94 @@ def test_difference_is_bit_exact(N, offset):
         assert np.array_equal(got, ref)
     finally:
         toi.toi_plan_destroy(plan)
+
+
+# ------------------------------------------------------------------------------------------------
+# output side of the streamed run (interpolate + copy_cpu stages)
+# ------------------------------------------------------------------------------------------------
+def _stream_case(n=6, ring=3):
+    import ctypes as C
+    wl = synth.reduced(synth.CONFIG5, n_ant=12, n_core=9, n_chan=48, image_size=128, dt_s=120.0)
+    snaps = [snapshot_np(wl, k) for k in range(n)]
+    plan = toi.toi_plan_create(wl.n_baselines, wl.n_chan, wl.n_pol, snaps[0]["chan_freq_hz"], wl.image_size,
+                               wl.cell_size_deg, pol_a=0, pol_b=3, input_location=toi.TOI_MEM_HOST,
+                               image_ring_depth=ring)
+
+    def fill(idx, slot):
+        s = snaps[idx]
+        for name, ptr in (("uvw_m", slot.uvw_m), ("vis", slot.vis), ("weights", slot.weights), ("flags", slot.flags)):
+            a = np.ascontiguousarray(s[name])
+            C.memmove(ptr, a.ctypes.data, a.nbytes)
+        return 0
+
+    refs = []
+    for s in snaps:
+        rc, img_o, info_o, _ = oracle.image_gridded(s["uvw_m"], s["vis"], s["weights"], s["flags"], s["chan_freq_hz"],
+                                                    wl.image_size, wl.cell_size_deg, pol_a=0, pol_b=3)
+        assert rc == 0
+        refs.append((img_o, info_o["V"]))
+    return wl, plan, fill, refs
+
+
+def _close(got, ref, peak):
+    m = ~np.isnan(ref) & ~np.isnan(got)
+    assert (np.isnan(ref) != np.isnan(got)).mean() < 1e-3 and m.mean() > 0.2
+    assert float(np.max(np.abs(got[m] - ref[m]))) <= 1e-4 * peak
+
+
+@pytest.mark.parametrize("product,difference", [("tilted", False), ("exact", False), ("paper", True), ("tilted", True)])
+def test_stream_output_ring_delivers_every_image_to_the_host_in_order(product, difference):
+    n = 6
+    wl, plan, fill, refs = _stream_case(n)
+    N, cell = wl.image_size, wl.cell_size_deg
+    code = {"tilted": toi.TOI_OUT_TILTED, "exact": toi.TOI_OUT_REPROJECT_EXACT, "paper": toi.TOI_OUT_REPROJECT_PAPER}[product]
+    prods = [img if product == "tilted" else orp.reproject(img, V, cell, product) for img, V in refs]
+    host, dev = {}, {}
+
+    def host_sink(idx, image):
+        assert idx not in host and (not host or idx == max(host) + 1)      # in order, once
+        host[idx] = image.copy()
+
+    def sink(idx, d_image, stream, info):
+        dev[idx] = d_image
+
+    try:
+        toi.toi_stream_set_output(plan, product=code, difference=difference, host_sink=host_sink, image_size=N)
+        stats = toi.toi_image_stream(plan, n, fill, sink)
+        first = 1 if difference else 0
+        assert sorted(host) == list(range(first, n)) and sorted(dev) == list(range(n))
+        assert stats["d2h_bytes"] == (n - first) * N * N * 4 and stats["d2h_ms_sum"] > 0 and stats["gpu_ms"] > 0
+        peak = max(float(np.nanmax(np.abs(p))) for p in prods)
+        for k in range(first, n):
+            ref = orp.difference(prods[k], prods[k - 1]) if difference else prods[k]
+            _close(host[k].astype(np.float64), ref, peak)
+        # the last delivered device image is still in its ring / ping-pong buffer
+        last = toi.toi_copy_image_to_host(plan, dev[n - 1], N).numpy()
+        assert np.array_equal(np.nan_to_num(last, nan=-1.0), np.nan_to_num(host[n - 1], nan=-1.0))
+        # a second run on the same plan, default output restored: nothing reaches the host sink
+        host.clear()
+        toi.toi_stream_set_output(plan)
+        stats = toi.toi_image_stream(plan, 2, fill, sink)
+        assert not host and stats["d2h_bytes"] == 0
+    finally:
+        toi.toi_plan_destroy(plan)
+
+
+def test_stream_output_refuses_bad_settings_and_propagates_host_sink_errors():
+    wl, plan, fill, _ = _stream_case(3, ring=1)
+    try:
+        with pytest.raises(toi.ToiError) as ei:
+            toi.toi_stream_set_output(plan, difference=True)
+        assert ei.value.code == toi.TOI_ERR_INVALID_ARG          # ring depth 1
+        with pytest.raises(toi.ToiError):
+            toi.toi_stream_set_output(plan, product=9)
+    finally:
+        toi.toi_plan_destroy(plan)
+    wl, plan, fill, _ = _stream_case(4, ring=2)
+    try:
+        toi.toi_stream_set_output(plan, host_sink=lambda idx, image: -1, image_size=wl.image_size)
+        with pytest.raises(toi.ToiError) as ei:
+            toi.toi_image_stream(plan, 4, fill)
+        assert ei.value.code == toi.TOI_ERR_CALLBACK
+    finally:
+        toi.toi_plan_destroy(plan)
