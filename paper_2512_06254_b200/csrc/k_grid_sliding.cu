@@ -41,7 +41,7 @@ constexpr int kGroups = 4;        // 7-lane groups per warp
 constexpr int kBatch = 8;         // samples per group per pre-processing batch (4 * 8 = 32 lanes)
 constexpr int kWarps = 8;         // warps per CTA
 constexpr int kCtasPerSm = 3;     // resident CTAs per SM (80 registers per thread; 4 x 64 measured slower)
-constexpr int kRecQuads = 5;      // record = 5 x 16 B: {zre, zim, key, -} {pu0..3} {pu4..6, 0} {pv0..3} {pv4..6, 0}
+constexpr int kRecQuads = 5;      // record = 5 x 16 B: {zre, zim, key, pv0} {pv1..4} {pv5, pv6, 0, 0} {pu0..3} {pu4..6, 0}
 constexpr int kGroupQuads = kBatch * kRecQuads + 2;   // +32 B: groups land on distinct banks
 constexpr int kWarpQuads = kGroups * kGroupQuads;
 constexpr unsigned kNoKey = 0x80008000u;   // (iv, iu) = (-32768, -32768): never an on-grid cell
@@ -84,27 +84,27 @@ __device__ __forceinline__ void flush_col(const u64 (&a)[kW], const char *p, lon
 // a warp are split only while one of them moves its window), which slides or reopens the window
 // and reloads my phi_u tap.
 #define TOI_REC_HEAD(P, OFF)                                                                          \
-    "ld.shared.v4.b32 {zx" #P ", zy" #P ", key" #P ", pad}, [%11+" #OFF "];\n\t"                     \
+    "ld.shared.v4.b32 {zx" #P ", zy" #P ", key" #P ", va" #P "}, [%11+" #OFF "];\n\t"                \
     "ld.shared.b32 pw" #P ", [%10+" #OFF "];\n\t"
 #define TOI_REC_FMA(P)                                                                                \
     "mov.b64 tt, {zx" #P ", zy" #P "};\n\tmov.b64 bb, {pw" #P ", pw" #P "};\n\t"                     \
     "mul.rn.f32x2 tt, tt, bb;\n\t"                                                                    \
-    "mov.b64 bb, {v0, v0};\n\tfma.rn.f32x2 %0, tt, bb, %0;\n\t"                                       \
+    "mov.b64 bb, {va" #P ", va" #P "};\n\tfma.rn.f32x2 %0, tt, bb, %0;\n\t"                          \
     "mov.b64 bb, {v1, v1};\n\tfma.rn.f32x2 %1, tt, bb, %1;\n\t"                                       \
     "mov.b64 bb, {v2, v2};\n\tfma.rn.f32x2 %2, tt, bb, %2;\n\t"                                       \
     "mov.b64 bb, {v3, v3};\n\tfma.rn.f32x2 %3, tt, bb, %3;\n\t"                                       \
     "mov.b64 bb, {v4, v4};\n\tfma.rn.f32x2 %4, tt, bb, %4;\n\t"                                       \
     "mov.b64 bb, {v5, v5};\n\tfma.rn.f32x2 %5, tt, bb, %5;\n\t"                                       \
     "mov.b64 bb, {v6, v6};\n\tfma.rn.f32x2 %6, tt, bb, %6;\n\t"
-#define TOI_REC_TEST(K, P, OFF48, OFF64)                                                              \
-    "ld.shared.v4.b32 {v0, v1, v2, v3}, [%11+" #OFF48 "];\n\t"                                        \
-    "ld.shared.v4.b32 {v4, v5, v6, v7}, [%11+" #OFF64 "];\n\t"                                        \
+#define TOI_REC_TEST(K, P, OFF16, OFF32)                                                              \
+    "ld.shared.v4.b32 {v1, v2, v3, v4}, [%11+" #OFF16 "];\n\t"                                        \
+    "ld.shared.v2.b32 {v5, v6}, [%11+" #OFF32 "];\n\t"                                                \
     "setp.ne.u32 pq, key" #P ", %9;\n\t"                                                              \
     "@pq bra S" #K ";\n\t"                                                                            \
     "B" #K ":\n\t"
-#define TOI_REC(K, P, PN, OFF48, OFF64, OFFN)                                                         \
-    TOI_REC_TEST(K, P, OFF48, OFF64) TOI_REC_HEAD(PN, OFFN) TOI_REC_FMA(P)
-#define TOI_REC_LAST(K, P, OFF48, OFF64) TOI_REC_TEST(K, P, OFF48, OFF64) TOI_REC_FMA(P)
+#define TOI_REC(K, P, PN, OFF16, OFF32, OFFN)                                                         \
+    TOI_REC_TEST(K, P, OFF16, OFF32) TOI_REC_HEAD(PN, OFFN) TOI_REC_FMA(P)
+#define TOI_REC_LAST(K, P, OFF16, OFF32) TOI_REC_TEST(K, P, OFF16, OFF32) TOI_REC_FMA(P)
 #define TOI_FLUSH7(A0, A1, A2, A3, A4, A5, A6)                                                        \
     "mov.u64 q, %7;\n\tcvt.u64.u32 q1, %13;\n\t"                                                     \
     "mov.b64 {x, y}, " A0 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
@@ -114,9 +114,9 @@ __device__ __forceinline__ void flush_col(const u64 (&a)[kW], const char *p, lon
     "mov.b64 {x, y}, " A4 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
     "mov.b64 {x, y}, " A5 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\tadd.s64 q, q, q1;\n\t"          \
     "mov.b64 {x, y}, " A6 ";\n\tred.global.add.v2.f32 [q], {x, y};\n\t"                               \
-    "mov.b64 " A0 ", {pad, pad};\n\tmov.b64 " A1 ", {pad, pad};\n\tmov.b64 " A2 ", {pad, pad};\n\t"   \
-    "mov.b64 " A3 ", {pad, pad};\n\tmov.b64 " A4 ", {pad, pad};\n\tmov.b64 " A5 ", {pad, pad};\n\t"   \
-    "mov.b64 " A6 ", {pad, pad};\n\t"
+    "@pz mov.b64 " A0 ", {pad, pad};\n\t@pz mov.b64 " A1 ", {pad, pad};\n\t@pz mov.b64 " A2 ", {pad, pad};\n\t"   \
+    "@pz mov.b64 " A3 ", {pad, pad};\n\t@pz mov.b64 " A4 ", {pad, pad};\n\t@pz mov.b64 " A5 ", {pad, pad};\n\t"   \
+    "@pz mov.b64 " A6 ", {pad, pad};\n\t"
 // The window of my group moves to the cell in key<P> (record K):
 //   * "no sample" record (padding / off-grid): nothing moves;
 //   * near move, (du, dv) each in {-1, 0, 1}: the lane that holds the retiring column flushes its 7
@@ -124,10 +124,17 @@ __device__ __forceinline__ void flush_col(const u64 (&a)[kW], const char *p, lon
 //     row accumulators by one register;
 //   * first sample of the strip, or a move by more than one cell: every lane flushes its column
 //     (if the window was open) and the window reopens at (cu, cv).
-// Flushes are red.global.add.v2.f32; freed accumulators are cleared from `pad`, the always-zero
-// fourth word of a record header (an immediate zero makes ptxas stage it through uniform registers).
+// Flushes are red.global.add.v2.f32; freed accumulators are cleared from `pad`, an always-zero
+// word of the records read once per batch (an immediate zero makes ptxas stage it through uniform
+// registers).
+// EVERY write to an accumulator in these blocks is predicated on pz = (pad == 0), which is always
+// true but opaque to ptxas: a predicated write must leave the old value in place when the predicate
+// is false, so the accumulator cannot be renamed across the block.  With plain writes ptxas joined
+// the fast path to the block's register assignment by 10 MOVs per record (24 -> 13 instructions
+// per record body once they are gone).
 #define TOI_SLOW(K, P, OFF)                                                                           \
     "S" #K ":\n\t"                                                                                    \
+    "setp.eq.u32 pz, pad, 0;\n\t"                                                                     \
     "setp.eq.u32 p0, key" #P ", 0x80008000;\n\t"                                                      \
     "@p0 bra B" #K ";\n\t"                                                                            \
     "shl.b32 t1, key" #P ", 16;\n\tshr.s32 cu, t1, 16;\n\tshr.s32 cv, key" #P ", 16;\n\t"            \
@@ -159,18 +166,18 @@ __device__ __forceinline__ void flush_col(const u64 (&a)[kW], const char *p, lon
     "@!pu bra NU" #K ";\n\t"                                                                          \
     "mov.b64 {x, y}, %0;\n\t"                                                                         \
     "red.global.add.v2.f32 [%7], {x, y};\n\t"                                                         \
-    "mul.rn.f32x2 %0, %1, one2;\n\tmul.rn.f32x2 %1, %2, one2;\n\tmul.rn.f32x2 %2, %3, one2;\n\t"      \
-    "mul.rn.f32x2 %3, %4, one2;\n\tmul.rn.f32x2 %4, %5, one2;\n\tmul.rn.f32x2 %5, %6, one2;\n\t"      \
-    "mov.b64 %6, {pad, pad};\n\t"                                                                   \
+    "@pz mul.rn.f32x2 %0, %1, one2;\n\t@pz mul.rn.f32x2 %1, %2, one2;\n\t@pz mul.rn.f32x2 %2, %3, one2;\n\t"      \
+    "@pz mul.rn.f32x2 %3, %4, one2;\n\t@pz mul.rn.f32x2 %4, %5, one2;\n\t@pz mul.rn.f32x2 %5, %6, one2;\n\t"      \
+    "@pz mov.b64 %6, {pad, pad};\n\t"                                                                   \
     "mad.wide.u32 %7, %13, 1, %7;\n\t"                                                                \
     "NU" #K ":\n\t"                                                                                   \
     "@!pd bra F" #K ";\n\t"                                                                           \
     "mad.wide.u32 q, %13, 6, %7;\n\t"                                                                 \
     "mov.b64 {x, y}, %6;\n\t"                                                                         \
     "red.global.add.v2.f32 [q], {x, y};\n\t"                                                          \
-    "mul.rn.f32x2 %6, %5, one2;\n\tmul.rn.f32x2 %5, %4, one2;\n\tmul.rn.f32x2 %4, %3, one2;\n\t"      \
-    "mul.rn.f32x2 %3, %2, one2;\n\tmul.rn.f32x2 %2, %1, one2;\n\tmul.rn.f32x2 %1, %0, one2;\n\t"      \
-    "mov.b64 %0, {pad, pad};\n\t"                                                                   \
+    "@pz mul.rn.f32x2 %6, %5, one2;\n\t@pz mul.rn.f32x2 %5, %4, one2;\n\t@pz mul.rn.f32x2 %4, %3, one2;\n\t"      \
+    "@pz mul.rn.f32x2 %3, %2, one2;\n\t@pz mul.rn.f32x2 %2, %1, one2;\n\t@pz mul.rn.f32x2 %1, %0, one2;\n\t"      \
+    "@pz mov.b64 %0, {pad, pad};\n\t"                                                                   \
     "cvt.u64.u32 q1, %13;\n\tsub.s64 %7, %7, q1;\n\t"                                                 \
     "bra F" #K ";\n\t"                                                                                \
     "O" #K ":\n\t"                                                                                    \
@@ -189,7 +196,7 @@ __device__ __forceinline__ void flush_col(const u64 (&a)[kW], const char *p, lon
     "F" #K ":\n\t"                                                                                    \
     "mov.u32 %9, key" #P ";\n\t"                                                                      \
     "shl.b32 t1, %8, 2;\n\t"                                                                          \
-    "add.u32 t1, t1, 16;\n\t"                                                                         \
+    "add.u32 t1, t1, 48;\n\t"                                                                         \
     "add.u32 %10, %11, t1;\n\t"                                                                       \
     "ld.shared.b32 pw" #P ", [%10+" #OFF "];\n\t"                                                     \
     "bra B" #K ";\n\t"
@@ -200,20 +207,21 @@ __device__ __forceinline__ void consume_batch(u64 (&a)[kW], const char *&pcol, i
 {
     asm volatile(
         "{\n\t"
-        ".reg .b32 zx0, zy0, key0, pw0, zx1, zy1, key1, pw1, pad, v0, v1, v2, v3, v4, v5, v6, v7;\n\t"
+        ".reg .b32 zx0, zy0, key0, va0, pw0, zx1, zy1, key1, va1, pw1, pad, v1, v2, v3, v4, v5, v6;\n\t"
         ".reg .b32 t1, t2, cu, cv, ou, ov, du, dv;\n\t"
         ".reg .b64 tt, bb, one2, q, q1;\n\t"
         ".reg .f32 x, y;\n\t"
-        ".reg .pred pq, p0, po, pn, pc, pf, pu, pd;\n\t"
+        ".reg .pred pq, p0, po, pn, pc, pf, pu, pd, pz;\n\t"
+        "ld.shared.b32 pad, [%11+40];\n\t"      /* the always-zero third word of a record's third quad */
         TOI_REC_HEAD(0, 0)
-        TOI_REC(0, 0, 1, 48, 64, 80)
-        TOI_REC(1, 1, 0, 128, 144, 160)
-        TOI_REC(2, 0, 1, 208, 224, 240)
-        TOI_REC(3, 1, 0, 288, 304, 320)
-        TOI_REC(4, 0, 1, 368, 384, 400)
-        TOI_REC(5, 1, 0, 448, 464, 480)
-        TOI_REC(6, 0, 1, 528, 544, 560)
-        TOI_REC_LAST(7, 1, 608, 624)
+        TOI_REC(0, 0, 1, 16, 32, 80)
+        TOI_REC(1, 1, 0, 96, 112, 160)
+        TOI_REC(2, 0, 1, 176, 192, 240)
+        TOI_REC(3, 1, 0, 256, 272, 320)
+        TOI_REC(4, 0, 1, 336, 352, 400)
+        TOI_REC(5, 1, 0, 416, 432, 480)
+        TOI_REC(6, 0, 1, 496, 512, 560)
+        TOI_REC_LAST(7, 1, 576, 592)
         "bra DONE;\n\t"
         // ---------------- out of line: one window-move block per record ----------------
         TOI_SLOW(0, 0, 0)
@@ -330,7 +338,7 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
         unsigned ckey = kNoKey;              // closed window; else the packed centre cell (cu, cv)
         int mydu = 0;                        // which tap column of the window this lane holds
         const char *pcol = nullptr;          // &grid[cv - 3][cu - 3 + mydu]: top of my column
-        unsigned rpu = rgs + 16;             // shared address of my phi_u tap in record 0
+        unsigned rpu = rgs + 48;             // shared address of my phi_u tap in record 0
         float wpart = 0.0f;
 
         Raw nxt;
@@ -346,7 +354,7 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
                     load_raw<MODE>(g, in, has_w, has_f, q_row + c + kBatch, c + kBatch, nxt);
                 unsigned key = kNoKey;
                 bool valid = false;
-                float wI = 0.0f, zx = 0.0f, zy = 0.0f, dens = 1.0f;
+                float wI = 0.0f, zx = 0.0f, zy = 0.0f, dens = 1.0f, pv0 = 0.0f;
                 if (c < c_hi) {
                     int iu, iv;
                     float xu, xv;
@@ -373,10 +381,11 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
                             if (wb > 0.0f) { zx = fmaf(wb, cur.b.x, zx); zy = fmaf(wb, cur.b.y, zy); }
                             float pu[kW], pv[kW];
                             kernel_taps2(xu, xv, pu, pv);
-                            my_rec[1] = make_uint4(__float_as_uint(pu[0]), __float_as_uint(pu[1]), __float_as_uint(pu[2]), __float_as_uint(pu[3]));
-                            my_rec[2] = make_uint4(__float_as_uint(pu[4]), __float_as_uint(pu[5]), __float_as_uint(pu[6]), 0u);
-                            my_rec[3] = make_uint4(__float_as_uint(pv[0]), __float_as_uint(pv[1]), __float_as_uint(pv[2]), __float_as_uint(pv[3]));
-                            my_rec[4] = make_uint4(__float_as_uint(pv[4]), __float_as_uint(pv[5]), __float_as_uint(pv[6]), 0u);
+                            pv0 = pv[0];
+                            my_rec[1] = make_uint4(__float_as_uint(pv[1]), __float_as_uint(pv[2]), __float_as_uint(pv[3]), __float_as_uint(pv[4]));
+                            my_rec[2] = make_uint4(__float_as_uint(pv[5]), __float_as_uint(pv[6]), 0u, 0u);
+                            my_rec[3] = make_uint4(__float_as_uint(pu[0]), __float_as_uint(pu[1]), __float_as_uint(pu[2]), __float_as_uint(pu[3]));
+                            my_rec[4] = make_uint4(__float_as_uint(pu[4]), __float_as_uint(pu[5]), __float_as_uint(pu[6]), 0u);
                         }
                     }
                 }
@@ -387,7 +396,7 @@ k_grid_sliding(Geometry g, Inputs in, SnapState *__restrict__ st, const float *_
                 float f = 1.0f;
                 if (has_d) asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(f) : "f"(dens));
                 wpart = fmaf(f, wI, wpart);
-                my_rec[0] = make_uint4(__float_as_uint(zx * f), __float_as_uint(zy * f), key, 0u);
+                my_rec[0] = make_uint4(__float_as_uint(zx * f), __float_as_uint(zy * f), key, __float_as_uint(pv0));
             }
             __syncwarp();
             // ---------------- accumulate: group grp consumes its 8 records ----------------

@@ -17,8 +17,9 @@
 // neighbouring threads fall in the same or adjacent 128-B lines and are served by L1 -- writes
 // N^2 x 4 B).  Coordinates are fp64 (a pixel position must be good to ~1e-7 px at N = 8192, which
 // fp32 cannot hold); the row/column-separable parts are hoisted (per-thread column terms, per-row
-// terms once), leaving one fp64 sqrt, one fp64 divide and a handful of DFMA per pixel.  One thread
-// makes 4 consecutive pixels of a row and stores them as one 16-byte vector.
+// terms once); the square root and the quotient of Eq. 13 are fp32 MUFU seeds refined by one Newton
+// step in fp64 (no library slow paths): ~20 fp64 instructions per pixel.  One thread makes 4
+// consecutive pixels of a row and stores them as one 16-byte vector.
 #include <math_constants.h>
 
 #include "toi_internal.cuh"
@@ -31,14 +32,29 @@ struct Map {
     int ok;
 };
 
+// 1/d for d in [1e-6, 4]: fp32 MUFU seed (rel. error ~2^-23) + Newton steps in fp64 (each squares
+// the error); no special cases can occur in that range, so none of the library division's slow
+// paths are carried along.
+template <int STEPS>
+__device__ __forceinline__ double rcp_newton(double d)
+{
+    float r0;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"((float)d));
+    double r = (double)r0;
+#pragma unroll
+    for (int k = 0; k < STEPS; ++k) r = fma(r, fma(-d, r, 1.0), r);
+    return r;
+}
+
 __device__ __forceinline__ Map make_map(const double *V, int mode, int status)
 {
     Map M;
     M.ok = status == TOI_OK;
     if (mode == TOI_REPROJECT_PAPER) {
-        const double xi = V[6] / V[8], eta = V[7] / V[8];          // Eq. 14
-        M.m[0] = 1.0; M.m[1] = 0.0; M.m[2] = xi;
-        M.m[3] = 0.0; M.m[4] = 1.0; M.m[5] = eta;
+        const double r33 = M.ok ? rcp_newton<3>(fabs(V[8])) : 0.0;     // |V33| >= 1e-6 when ok
+        const double s33 = V[8] < 0.0 ? -r33 : r33;
+        M.m[0] = 1.0; M.m[1] = 0.0; M.m[2] = V[6] * s33;               // Eq. 14: xi
+        M.m[3] = 0.0; M.m[4] = 1.0; M.m[5] = V[7] * s33;               //         eta
     } else {
         M.m[0] = V[0]; M.m[1] = V[1]; M.m[2] = -V[2];
         M.m[3] = V[3]; M.m[4] = V[4]; M.m[5] = -V[5];
@@ -46,18 +62,30 @@ __device__ __forceinline__ Map make_map(const double *V, int mode, int status)
     return M;
 }
 
-__device__ __forceinline__ float sample_bilinear(const float *__restrict__ src, int N, double p1, double p2, bool valid)
+// Eq. 13, z = 1 - n = q / (1 + sqrt(1 - q)) for 0 <= q <= 1, relative error ~1e-13 (one Newton
+// step on an fp32 rsqrt seed gives n to ~1.5 e0^2 = 1e-13, one on an fp32 rcp seed the quotient):
+// z / beta is at most ~1e4 pixels, so the position is good to 1e-9 px.
+__device__ __forceinline__ double sin_z(double q)
 {
-    const double hi = (double)(N - 1), eps = 1e-6;
-    if (!(valid && p1 >= -eps && p1 <= hi + eps && p2 >= -eps && p2 <= hi + eps)) return CUDART_NAN_F;
-    p1 = fmin(fmax(p1, 0.0), hi);
-    p2 = fmin(fmax(p2, 0.0), hi);
-    const int i0 = min((int)p1, N - 2), j0 = min((int)p2, N - 2);   // p >= 0: truncation is floor
-    const float fx = (float)(p1 - (double)i0), fy = (float)(p2 - (double)j0);
-    const float *r0 = src + (size_t)j0 * N + i0, *r1 = r0 + N;
-    const float a = __ldg(r0), b = __ldg(r0 + 1), c = __ldg(r1), d = __ldg(r1 + 1);
-    const float top = fmaf(fx, b - a, a), bot = fmaf(fx, d - c, c);
-    return fmaf(fy, bot - top, top);
+    const double a = fmax(1.0 - q, 1e-30);                 // a -> 0 at the horizon: n -> 0
+    float y0f;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0f) : "f"((float)a));
+    const double y0 = (double)y0f;
+    const double t = a * y0;                               // ~ sqrt(a)
+    const double n = fma(0.5 * t, fma(-t, y0, 1.0), t);    // Newton: t (1 + (1 - a y0^2)/2)
+    return q * rcp_newton<1>(1.0 + n);
+}
+
+// One axis of the bilinear tap: p -> first neighbour i0 in [0, N-2] and weight f in [0, 1] of the
+// second; false when p is more than 1e-6 px outside [0, N-1] (G22).
+__device__ __forceinline__ bool tap(double p, int N, int &i0, float &f)
+{
+    const int k = __double2int_rd(p);
+    const float w = (float)(p - (double)k);
+    const bool lo = k == -1 && w >= 1.0f - 1e-6f, hi = k == N - 1 && w <= 1e-6f;
+    i0 = lo ? 0 : (hi ? N - 2 : k);
+    f = lo ? 0.0f : (hi ? 1.0f : w);
+    return (unsigned)k < (unsigned)(N - 1) || lo || hi;
 }
 
 template <int PIX>
@@ -72,18 +100,28 @@ k_reproject(int N, double beta_rad, const SnapState *__restrict__ st, const doub
     const double inv_beta = 1.0 / beta_rad, half = (double)(N >> 1);
     const double m_ = beta_rad * (double)(j - (N >> 1));
     const double mm = m_ * m_, r1 = M.m[1] * m_, r2 = M.m[4] * m_;
+    const double l0 = -beta_rad * (double)(i_base - (N >> 1));
     float out[PIX];
 #pragma unroll
     for (int k = 0; k < PIX; ++k) {
-        const int i = i_base + k;
-        const double l = -beta_rad * (double)(i - (N >> 1));
+        const double l = fma(-beta_rad, (double)k, l0);
         const double q = fma(l, l, mm);
-        const bool valid = M.ok && q <= 1.0 && i < N;
-        const double qs = valid ? q : 0.0;
-        const double z = qs / (1.0 + sqrt(1.0 - qs));                 // Eq. 13: 1 - n
+        const double z = sin_z(fmin(q, 1.0));
         const double t1 = fma(M.m[2], z, fma(M.m[0], l, r1));
         const double t2 = fma(M.m[5], z, fma(M.m[3], l, r2));
-        out[k] = sample_bilinear(src, N, fma(-t1, inv_beta, half), fma(t2, inv_beta, half), valid);
+        int i0, j0;
+        float fx, fy;
+        bool ok = M.ok && q <= 1.0 && i_base + k < N;
+        ok = tap(fma(-t1, inv_beta, half), N, i0, fx) && ok;
+        ok = tap(fma(t2, inv_beta, half), N, j0, fy) && ok;
+        float v = CUDART_NAN_F;
+        if (ok) {
+            const float *p0 = src + (size_t)j0 * N + i0, *p1 = p0 + N;
+            const float a = __ldg(p0), b = __ldg(p0 + 1), c = __ldg(p1), d = __ldg(p1 + 1);
+            const float top = fmaf(fx, b - a, a), bot = fmaf(fx, d - c, c);
+            v = fmaf(fy, bot - top, top);
+        }
+        out[k] = v;
     }
     float *o = dst + (size_t)j * N + i_base;
     if (PIX == 4) {
