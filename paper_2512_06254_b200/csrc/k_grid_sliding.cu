@@ -252,6 +252,8 @@ struct Raw {
 // MODE 4: n_p = 4, hands (0, 3), 16-B aligned weights and 4-B aligned flags -> 2 LDG.64 + LDG.128 + LDG.32
 // MODE 2: n_p = 2, hands (0, 1), 8-B aligned weights, 2-B aligned flags     -> LDG.128 + LDG.64 + LDG.U16
 // MODE 0: anything else, scalar loads
+// The raw inputs are read exactly once: __ldcs (evict-first) keeps them from displacing the density
+// lines and the channel-scale table, which ARE re-read, from L1/L2.
 template <int MODE>
 __device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, bool has_w, bool has_f,
                                          long long q, int c, Raw &r)
@@ -261,28 +263,28 @@ __device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, bo
     r.fl = 0u;
     if (MODE == 4) {
         const float2 *v = in.vis + 4 * q;
-        r.a = __ldg(v);
-        r.b = __ldg(v + 3);
+        r.a = __ldcs(v);
+        r.b = __ldcs(v + 3);
         if (has_w) {
-            const float4 w = __ldg(reinterpret_cast<const float4 *>(in.weights) + q);
+            const float4 w = __ldcs(reinterpret_cast<const float4 *>(in.weights) + q);
             r.wa = w.x; r.wb = w.w;
         }
-        if (has_f) r.fl = __ldg(reinterpret_cast<const unsigned *>(in.flags) + q);
+        if (has_f) r.fl = __ldcs(reinterpret_cast<const unsigned *>(in.flags) + q);
     } else if (MODE == 2) {
-        const float4 v = __ldg(reinterpret_cast<const float4 *>(in.vis) + q);
+        const float4 v = __ldcs(reinterpret_cast<const float4 *>(in.vis) + q);
         r.a = make_float2(v.x, v.y);
         r.b = make_float2(v.z, v.w);
         if (has_w) {
-            const float2 w = __ldg(reinterpret_cast<const float2 *>(in.weights) + q);
+            const float2 w = __ldcs(reinterpret_cast<const float2 *>(in.weights) + q);
             r.wa = w.x; r.wb = w.y;
         }
-        if (has_f) r.fl = __ldg(reinterpret_cast<const unsigned short *>(in.flags) + q);
+        if (has_f) r.fl = __ldcs(reinterpret_cast<const unsigned short *>(in.flags) + q);
     } else {
         const long long o = q * g.n_p;
-        r.a = __ldg(in.vis + o + g.pol_a);
-        r.b = __ldg(in.vis + o + g.pol_b);
-        if (has_w) { r.wa = __ldg(in.weights + o + g.pol_a); r.wb = __ldg(in.weights + o + g.pol_b); }
-        if (has_f) r.fl = (unsigned)__ldg(in.flags + o + g.pol_a) | ((unsigned)__ldg(in.flags + o + g.pol_b) << 24);
+        r.a = __ldcs(in.vis + o + g.pol_a);
+        r.b = __ldcs(in.vis + o + g.pol_b);
+        if (has_w) { r.wa = __ldcs(in.weights + o + g.pol_a); r.wb = __ldcs(in.weights + o + g.pol_b); }
+        if (has_f) r.fl = (unsigned)__ldcs(in.flags + o + g.pol_a) | ((unsigned)__ldcs(in.flags + o + g.pol_b) << 24);
         if (g.pol_b == g.pol_a) r.fl |= 0xff000000u;     // single hand: b never contributes
     }
 }
@@ -447,11 +449,8 @@ void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, con
     // end, short ones balance the persistent grid's tail.  Aim at >= 6 tasks per resident warp,
     // within [32, 256] channels and a multiple of the 8-sample batch.
     const long long warps = (long long)kCtasPerSm * n_sms * kWarps;
-    long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
-    want = want / kBatch * kBatch;
-    int strip = (int)(want < 32 ? 32 : (want > 256 ? 256 : want));
-    const int quarter = ((g.n_c + kGroups - 1) / kGroups + kBatch - 1) / kBatch * kBatch;
-    if (strip > quarter) strip = quarter;
+    const long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
+    int strip = pick_strip(g.n_c, kGroups, kBatch, want, 32, 256);
     if (const char *e = getenv("TOI_STRIP")) strip = atoi(e);   // tuning override (multiple of 8)
     const int tasks_per_row = (g.n_c + kGroups * strip - 1) / (kGroups * strip);
     const long long n_tasks = (long long)g.n_b * tasks_per_row;

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <cufft.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include "../../include/toi.h"
 
@@ -197,6 +198,27 @@ __device__ __forceinline__ void kernel_taps2(float xu, float xv, float pu[kW], f
 #undef TOI_PAIR
 }
 
+// Strip length of the sliding-window gridders: a task is `groups` strips of `strip` consecutive
+// channels of one baseline.  Near `want` (tasks per resident warp), a multiple of `batch`, and such
+// that the tasks of a row cover n_c with the least padding (a padded task still walks all its
+// batches): n_c = 4096 with 4 groups and want = 96 gives 104 (10 tasks, 1.5 % padding) instead of
+// 96 (11 tasks, 3 %); with 8 groups and want = 72 it gives 64 (8 tasks, none) instead of 72 (12 %).
+inline int pick_strip(int n_c, int groups, int batch, long long want, int lo, int hi)
+{
+    if (want < lo) want = lo;
+    if (want > hi) want = hi;
+    const int share = ((n_c + groups - 1) / groups + batch - 1) / batch * batch;   // one task per row
+    if (want >= share) return share;
+    int best = (int)(want / batch * batch), best_pad = 1 << 30;
+    for (int s = (int)(want * 3 / 4) / batch * batch; s <= want * 5 / 4; s += batch) {
+        if (s < lo || s > hi || s > share) continue;
+        const int t = (n_c + groups * s - 1) / (groups * s);
+        const int pad = t * groups * s - n_c;
+        if (pad < best_pad || (pad == best_pad && llabs(s - want) < llabs(best - want))) { best = s; best_pad = pad; }
+    }
+    return best;
+}
+
 // ---- host-side launchers, one per translation unit -------------------------------------------
 void launch_planefit(const Geometry &g, const double *d_uvw, double S1, double S2, const double *d_V_inject,
                      SnapState *st, cudaStream_t stream);
@@ -205,6 +227,8 @@ void launch_grid_atomic(const Geometry &g, const Inputs &in, SnapState *st, cons
                         float2 *d_grid, cudaStream_t stream);
 void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                          float2 *d_grid, int n_sms, cudaStream_t stream);
+void launch_grid_pair(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
+                      float2 *d_grid, int n_sms, cudaStream_t stream);
 void launch_correct_crop(const Geometry &g, const float2 *d_F, const double *d_ipsi, const SnapState *st,
                          int apply_jacobian, float *d_image, cudaStream_t stream);
 void launch_reproject(int N, double beta_rad, const SnapState *st, const double *d_V, int mode, const float *d_src,

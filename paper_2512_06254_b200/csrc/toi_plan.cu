@@ -237,8 +237,10 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     // a3 + a5: cell indices and gridding onto the zero-filled grid
     if (p->cfg.gridder == TOI_GRIDDER_ATOMIC)
         launch_grid_atomic(g, in, p->d_state, dens, grid, stream);
-    else
+    else if (p->cfg.gridder == TOI_GRIDDER_SLIDING7)
         launch_grid_sliding(g, in, p->d_state, dens, grid, p->n_sms, stream);
+    else
+        launch_grid_pair(g, in, p->d_state, dens, grid, p->n_sms, stream);
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev[EV_GRID], stream));
     if (p->keep_grid && p->d_grid_keep)
@@ -346,7 +348,8 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     if (W != kW) return fail(nullptr, TOI_ERR_UNSUPPORTED, "only kernel_support = 7 is built");
     if (cfg->weighting != TOI_WEIGHT_NATURAL && cfg->weighting != TOI_WEIGHT_UNIFORM) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown weighting");
     if (cfg->input_location != TOI_MEM_HOST && cfg->input_location != TOI_MEM_DEVICE) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown input_location");
-    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown gridder");
+    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC && cfg->gridder != TOI_GRIDDER_SLIDING7)
+        return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown gridder");
     if (cfg->image_ring_depth < 0 || cfg->image_ring_depth > 64) return fail(nullptr, TOI_ERR_INVALID_ARG, "image_ring_depth must be in [0, 64]");
     if (cfg->apply_jacobian < 0 || cfg->apply_jacobian > 2) return fail(nullptr, TOI_ERR_INVALID_ARG, "apply_jacobian must be 0, 1 or 2");
     for (int k = 0; k < 7; ++k)

@@ -93,7 +93,10 @@ def _check_all(snap, wl_N, cell, weighting, gridder, pol_a=None, pol_b=None, loc
 # ------------------------------------------------------------------------------------------------
 # config 1 (BASELINE.json configs[0]): the tiny snapshot, natural weighting, both gridders
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("gridder", [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_ATOMIC])
+ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_SLIDING7, toi.TOI_GRIDDER_ATOMIC]
+
+
+@pytest.mark.parametrize("gridder", ALL_GRIDDERS)
 def test_config1_natural(gridder):
     wl = synth.CONFIG1
     snap = snapshot_np(wl)
@@ -129,7 +132,7 @@ def _reduced2(n_ant=24, n_chan=777, image_size=512, **kw):
 
 
 @pytest.mark.parametrize("weighting", ["natural", "uniform"])
-@pytest.mark.parametrize("gridder", [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_ATOMIC])
+@pytest.mark.parametrize("gridder", ALL_GRIDDERS)
 def test_reduced_config2(weighting, gridder):
     wl = _reduced2()
     snap = snapshot_np(wl)
@@ -143,6 +146,17 @@ def test_reduced_config2_long_rows():
     snap = snapshot_np(wl)
     _check_all(snap, wl.image_size, wl.cell_size_deg, "natural", toi.TOI_GRIDDER_SLIDING, pol_a=0, pol_b=3,
                check_grid=False)
+
+
+@pytest.mark.parametrize("gridder", [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_SLIDING7])
+@pytest.mark.parametrize("weighting", ["natural", "uniform"])
+def test_coarse_channels_make_the_window_jump(gridder, weighting):
+    """16 channels across the whole band: consecutive samples of a long baseline are tens of cells
+    apart, so nearly every record takes the "far move" path (flush everything, reopen) instead of
+    sliding by one cell; short baselines still slide.  Also mixes diagonal moves."""
+    wl = _reduced2(n_ant=14, n_chan=16, image_size=1024)
+    snap = snapshot_np(wl)
+    _check_all(snap, wl.image_size, wl.cell_size_deg, weighting, gridder, pol_a=0, pol_b=3)
 
 
 def test_low_elevation_config5_shape():
@@ -180,7 +194,7 @@ def test_edge_single_pol_flags_nan_and_bad_weights():
     w[1, 3, 1] = -1.0
     w[2, 4, 0] = np.nan
     w[2, 5, 1] = np.inf
-    for gridder in (toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_ATOMIC):
+    for gridder in ALL_GRIDDERS:
         e, _ = _check_all(snap, wl.image_size, wl.cell_size_deg, "natural", gridder)
     _check_all(snap, wl.image_size, wl.cell_size_deg, "uniform", toi.TOI_GRIDDER_SLIDING)
 
@@ -191,7 +205,7 @@ def test_edge_off_grid_samples_dropped():
     cell = 3.0 * wl.cell_size_deg                  # grid half-extent shrinks 3x: long baselines fall off
     rc, _, info_o, _ = _oracle(snap, wl.image_size, cell)
     assert rc == 0 and info_o["n_off_grid"] > 0 and info_o["n_gridded"] > 0
-    for gridder in (toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_ATOMIC):
+    for gridder in ALL_GRIDDERS:
         _check_all(snap, wl.image_size, cell, "natural", gridder)
     _check_all(snap, wl.image_size, cell, "uniform", toi.TOI_GRIDDER_SLIDING)
 
