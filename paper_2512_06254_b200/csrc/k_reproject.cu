@@ -17,8 +17,9 @@
 // neighbouring threads fall in the same or adjacent 128-B lines and are served by L1 -- writes
 // N^2 x 4 B).  Coordinates are fp64 (a pixel position must be good to ~1e-7 px at N = 8192, which
 // fp32 cannot hold); the row/column-separable parts are hoisted (per-thread column terms, per-row
-// terms once); the square root and the quotient of Eq. 13 are fp32 MUFU seeds refined by one Newton
-// step in fp64 (no library slow paths): ~20 fp64 instructions per pixel.  One thread makes 4
+// terms once); the square root and the quotient of Eq. 13 are 20-bit MUFU.RSQ64H / RCP64H seeds refined
+// by one Newton step in fp64 (no library slow paths, no fp64<->fp32 conversions on the quarter-rate
+// XU pipe, which bounded the first version): ~26 fp64 instructions and 4 XU instructions per pixel.  One thread makes 4
 // consecutive pixels of a row and stores them as one 16-byte vector.
 #include <math_constants.h>
 
@@ -32,15 +33,15 @@ struct Map {
     int ok;
 };
 
-// 1/d for d in [1e-6, 4]: fp32 MUFU seed (rel. error ~2^-23) + Newton steps in fp64 (each squares
-// the error); no special cases can occur in that range, so none of the library division's slow
-// paths are carried along.
+// 1/d for d in [1e-6, 4]: MUFU.RCP64H seed (rcp.approx.ftz.f64: ~20 good bits from ONE instruction of
+// the quarter-rate XU pipe, where an fp32 seed costs three -- two conversions and the MUFU) + Newton
+// steps in fp64 (each squares the error); no special cases can occur in that range, so none of the
+// library division's slow paths are carried along.
 template <int STEPS>
 __device__ __forceinline__ double rcp_newton(double d)
 {
-    float r0;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"((float)d));
-    double r = (double)r0;
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
 #pragma unroll
     for (int k = 0; k < STEPS; ++k) r = fma(r, fma(-d, r, 1.0), r);
     return r;
@@ -51,7 +52,7 @@ __device__ __forceinline__ Map make_map(const double *V, int mode, int status)
     Map M;
     M.ok = status == TOI_OK;
     if (mode == TOI_REPROJECT_PAPER) {
-        const double r33 = M.ok ? rcp_newton<3>(fabs(V[8])) : 0.0;     // |V33| >= 1e-6 when ok
+        const double r33 = M.ok ? rcp_newton<4>(fabs(V[8])) : 0.0;     // |V33| >= 1e-6 when ok
         const double s33 = V[8] < 0.0 ? -r33 : r33;
         M.m[0] = 1.0; M.m[1] = 0.0; M.m[2] = V[6] * s33;               // Eq. 14: xi
         M.m[3] = 0.0; M.m[4] = 1.0; M.m[5] = V[7] * s33;               //         eta
@@ -62,30 +63,34 @@ __device__ __forceinline__ Map make_map(const double *V, int mode, int status)
     return M;
 }
 
-// Eq. 13, z = 1 - n = q / (1 + sqrt(1 - q)) for 0 <= q <= 1, relative error ~1e-13 (one Newton
-// step on an fp32 rsqrt seed gives n to ~1.5 e0^2 = 1e-13, one on an fp32 rcp seed the quotient):
-// z / beta is at most ~1e4 pixels, so the position is good to 1e-9 px.
+// Eq. 13, z = 1 - n = q / (1 + sqrt(1 - q)) for 0 <= q <= 1, relative error ~2e-12 (one Newton
+// step on a 20-bit MUFU.RSQ64H seed gives n to 1.5 e0^2, one on a MUFU.RCP64H seed the quotient):
+// z / beta is at most ~1e4 pixels, so the position is good to ~1e-8 px.
 __device__ __forceinline__ double sin_z(double q)
 {
-    const double a = fmax(1.0 - q, 1e-30);                 // a -> 0 at the horizon: n -> 0
-    float y0f;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0f) : "f"((float)a));
-    const double y0 = (double)y0f;
+    // + 1e-300: a stays a positive normal number at the horizon (q = 1: n -> 0, z -> 1) and is
+    // unchanged everywhere else; q > 1 (outside the SIN domain) gives NaN, which the caller never uses
+    const double a = (1.0 - q) + 1e-300;
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(a));
     const double t = a * y0;                               // ~ sqrt(a)
     const double n = fma(0.5 * t, fma(-t, y0, 1.0), t);    // Newton: t (1 + (1 - a y0^2)/2)
     return q * rcp_newton<1>(1.0 + n);
 }
 
 // One axis of the bilinear tap: p -> first neighbour i0 in [0, N-2] and weight f in [0, 1] of the
-// second; false when p is more than 1e-6 px outside [0, N-1] (G22).
+// second; false when p is more than 1e-6 px outside [0, N-1] (G22) or NaN.  floor(p) by the
+// magic-number add (round-down add of 2^52 + 2^51 leaves floor(p) in the low word) on the fp64
+// pipe instead of two XU conversions; its result is only used when the range test passed.
 __device__ __forceinline__ bool tap(double p, int N, int &i0, float &f)
 {
-    const int k = __double2int_rd(p);
-    const float w = (float)(p - (double)k);
-    const bool lo = k == -1 && w >= 1.0f - 1e-6f, hi = k == N - 1 && w <= 1e-6f;
-    i0 = lo ? 0 : (hi ? N - 2 : k);
-    f = lo ? 0.0f : (hi ? 1.0f : w);
-    return (unsigned)k < (unsigned)(N - 1) || lo || hi;
+    const bool in = p >= -1e-6 && p <= (double)(N - 1) + 1e-6;       // false for NaN
+    const double m = __dadd_rd(p, kFloorMagic);
+    const int k = __double2loint(m);                                 // -1 .. N-1 when in
+    const float w = (float)(p - (m - kFloorMagic));                  // [0, 1)
+    i0 = min(max(k, 0), N - 2);
+    f = k < 0 ? 0.0f : (k > N - 2 ? 1.0f : w);
+    return in;
 }
 
 template <int PIX>
