@@ -41,7 +41,7 @@ def parse_args():
     ap.add_argument("--workload", type=int, default=2, choices=[1, 2, 4, 5],
                     help="BASELINE.json config id (2 = configs[1], the metric's workload)")
     ap.add_argument("--weighting", default=None, choices=[None, "natural", "uniform"])
-    ap.add_argument("--gridder", default="sliding", choices=["sliding", "sliding7", "atomic"])
+    ap.add_argument("--gridder", default="sliding", choices=["sliding", "pair7", "sliding7", "atomic"])
     ap.add_argument("--stream-snapshots", type=int, default=60,
                     help="length of the streamed (config-3-shaped) run reported under `stream`; 0 = skip")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -210,7 +210,7 @@ def run_ours(args):
     toi.load()
     wl, weighting = workload(args)
     wt = toi.TOI_WEIGHT_UNIFORM if weighting == "uniform" else toi.TOI_WEIGHT_NATURAL
-    gridder = {"sliding": toi.TOI_GRIDDER_SLIDING, "sliding7": toi.TOI_GRIDDER_SLIDING7,
+    gridder = {"sliding": toi.TOI_GRIDDER_SLIDING, "pair7": toi.TOI_GRIDDER_PAIR7, "sliding7": toi.TOI_GRIDDER_SLIDING7,
                "atomic": toi.TOI_GRIDDER_ATOMIC}[args.gridder]
     S = wl.n_baselines * wl.n_chan
     N = wl.image_size
@@ -437,7 +437,7 @@ def main():
     zero_alone_ms = r["zero_alone_ms"]
     grid_ms = r["stages"]["ms_grid"] + zero_alone_ms
     achieved = ab["gridding"] / (grid_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "%s (+ grid zero fill on the side stream)" % {"sliding": "k_grid_pair", "sliding7": "k_grid_sliding", "atomic": "k_grid_atomic"}[args.gridder], "achieved": achieved,
+    roofline = {"bound": "hbm", "kernel": "%s (+ grid zero fill on the side stream)" % {"sliding": "k_grid_pair8", "pair7": "k_grid_pair", "sliding7": "k_grid_sliding", "atomic": "k_grid_atomic"}[args.gridder], "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_8tbs_nominal": achieved / 8000.0,
                 "peak_source": peak_src, "traffic": ncu_traffic(args, weighting),
                 "algorithmic_bytes": ab["gridding"], "ms": grid_ms, "ms_kernel": r["stages"]["ms_grid"],

@@ -52,7 +52,7 @@ enum { TOI_MEM_HOST = 0, TOI_MEM_DEVICE = 1 };
  * columns per lane, k_grid_pair.cu); SLIDING7 is its predecessor (groups of 7 lanes, one column per
  * lane, k_grid_sliding.cu), kept for comparison; ATOMIC (one thread per sample, 98 global float
  * atomics) is the ncu comparison point the design replaces. */
-enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1, TOI_GRIDDER_SLIDING7 = 2 };
+enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1, TOI_GRIDDER_SLIDING7 = 2, TOI_GRIDDER_PAIR7 = 3 };
 
 /* The paper's inputs (Measurement Set, image size, cell size) plus the knobs the
  * paper leaves open.  Zero selects the default of every optional field. */

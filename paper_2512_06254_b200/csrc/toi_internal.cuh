@@ -229,6 +229,11 @@ void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, con
                          float2 *d_grid, int n_sms, cudaStream_t stream);
 void launch_grid_pair(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                       float2 *d_grid, int n_sms, cudaStream_t stream);
+void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
+                       float2 *d_grid, int n_sms, cudaStream_t stream);
+// elements of guard band before and after the grid: k_grid_pair8's 8 x 8 window may overhang the
+// grid by one row / column (of zeros); a multiple of 32 elements keeps the grid 256-byte aligned
+inline size_t grid_guard(int G) { return ((size_t)G + 8 + 31) / 32 * 32; }
 void launch_correct_crop(const Geometry &g, const float2 *d_F, const double *d_ipsi, const SnapState *st,
                          int apply_jacobian, float *d_image, cudaStream_t stream);
 void launch_reproject(int N, double beta_rad, const SnapState *st, const double *d_V, int mode, const float *d_src,

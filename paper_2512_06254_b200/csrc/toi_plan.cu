@@ -44,6 +44,7 @@ struct toi_plan {
     // is zero-filled on s_zero for snapshot n + 1 (the fill is DRAM-write bound, the kernels it
     // runs under are issue bound)
     float2 *d_grids[2] = {nullptr, nullptr}, *d_grid_keep = nullptr;
+    float2 *d_grid_alloc[2] = {nullptr, nullptr};     // d_grids[k] = d_grid_alloc[k] + grid_guard(G)
     float *d_dens[2] = {nullptr, nullptr};
     cudaStream_t s_zero = nullptr;
     cudaEvent_t ev_zeroed[2] = {}, ev_free[2] = {}, ev_z0 = nullptr, ev_z1 = nullptr;
@@ -165,7 +166,7 @@ int free_plan(toi_plan *p)
         if (p->ev[k]) cudaEventDestroy(p->ev[k]);
     if (p->s_zero) cudaStreamSynchronize(p->s_zero);
     for (int k = 0; k < 2; ++k) {
-        cudaFree(p->d_grids[k]); cudaFree(p->d_dens[k]);
+        cudaFree(p->d_grid_alloc[k]); cudaFree(p->d_dens[k]);
         if (p->ev_zeroed[k]) cudaEventDestroy(p->ev_zeroed[k]);
         if (p->ev_free[k]) cudaEventDestroy(p->ev_free[k]);
     }
@@ -239,8 +240,10 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
         launch_grid_atomic(g, in, p->d_state, dens, grid, stream);
     else if (p->cfg.gridder == TOI_GRIDDER_SLIDING7)
         launch_grid_sliding(g, in, p->d_state, dens, grid, p->n_sms, stream);
-    else
+    else if (p->cfg.gridder == TOI_GRIDDER_PAIR7)
         launch_grid_pair(g, in, p->d_state, dens, grid, p->n_sms, stream);
+    else
+        launch_grid_pair8(g, in, p->d_state, dens, grid, p->n_sms, stream);
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev[EV_GRID], stream));
     if (p->keep_grid && p->d_grid_keep)
@@ -348,7 +351,8 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     if (W != kW) return fail(nullptr, TOI_ERR_UNSUPPORTED, "only kernel_support = 7 is built");
     if (cfg->weighting != TOI_WEIGHT_NATURAL && cfg->weighting != TOI_WEIGHT_UNIFORM) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown weighting");
     if (cfg->input_location != TOI_MEM_HOST && cfg->input_location != TOI_MEM_DEVICE) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown input_location");
-    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC && cfg->gridder != TOI_GRIDDER_SLIDING7)
+    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC && cfg->gridder != TOI_GRIDDER_SLIDING7 &&
+        cfg->gridder != TOI_GRIDDER_PAIR7)
         return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown gridder");
     if (cfg->image_ring_depth < 0 || cfg->image_ring_depth > 64) return fail(nullptr, TOI_ERR_INVALID_ARG, "image_ring_depth must be in [0, 64]");
     if (cfg->apply_jacobian < 0 || cfg->apply_jacobian > 2) return fail(nullptr, TOI_ERR_INVALID_ARG, "apply_jacobian must be 0, 1 or 2");
@@ -435,8 +439,11 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     CREATE_TRY(cudaEventCreate(&p->ev_z0));
     CREATE_TRY(cudaEventCreate(&p->ev_z1));
     for (int k = 0; k < 2; ++k) {
-        CREATE_TRY(cudaMalloc(&p->d_grids[k], GG * sizeof(float2)));
-        CREATE_TRY(cudaMemsetAsync(p->d_grids[k], 0, GG * sizeof(float2), p->s_zero));
+        // guard band on both sides: the gridder's 8 x 8 window may overhang the grid by one row or
+        // column of zero accumulators, whose flush must land in owned memory (never read)
+        CREATE_TRY(cudaMalloc(&p->d_grid_alloc[k], (GG + 2 * grid_guard(G)) * sizeof(float2)));
+        CREATE_TRY(cudaMemsetAsync(p->d_grid_alloc[k], 0, (GG + 2 * grid_guard(G)) * sizeof(float2), p->s_zero));
+        p->d_grids[k] = p->d_grid_alloc[k] + grid_guard(G);
         if (cfg->weighting == TOI_WEIGHT_UNIFORM) {
             CREATE_TRY(cudaMalloc(&p->d_dens[k], GG * sizeof(float)));
             CREATE_TRY(cudaMemsetAsync(p->d_dens[k], 0, GG * sizeof(float), p->s_zero));

@@ -93,7 +93,7 @@ def _check_all(snap, wl_N, cell, weighting, gridder, pol_a=None, pol_b=None, loc
 # ------------------------------------------------------------------------------------------------
 # config 1 (BASELINE.json configs[0]): the tiny snapshot, natural weighting, both gridders
 # ------------------------------------------------------------------------------------------------
-ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_SLIDING7, toi.TOI_GRIDDER_ATOMIC]
+ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_PAIR7, toi.TOI_GRIDDER_SLIDING7, toi.TOI_GRIDDER_ATOMIC]
 
 
 @pytest.mark.parametrize("gridder", ALL_GRIDDERS)
@@ -148,7 +148,7 @@ def test_reduced_config2_long_rows():
                check_grid=False)
 
 
-@pytest.mark.parametrize("gridder", [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_SLIDING7])
+@pytest.mark.parametrize("gridder", [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_PAIR7, toi.TOI_GRIDDER_SLIDING7])
 @pytest.mark.parametrize("weighting", ["natural", "uniform"])
 def test_coarse_channels_make_the_window_jump(gridder, weighting):
     """16 channels across the whole band: consecutive samples of a long baseline are tens of cells
