@@ -48,10 +48,11 @@ enum {
 
 enum { TOI_WEIGHT_NATURAL = 0, TOI_WEIGHT_UNIFORM = 1 };
 enum { TOI_MEM_HOST = 0, TOI_MEM_DEVICE = 1 };
-/* gridding kernels: SLIDING is the product (sliding 7x7 register window, groups of 4 lanes with two
- * columns per lane, k_grid_pair.cu); SLIDING7 is its predecessor (groups of 7 lanes, one column per
- * lane, k_grid_sliding.cu), kept for comparison; ATOMIC (one thread per sample, 98 global float
- * atomics) is the ncu comparison point the design replaces. */
+/* gridding kernels: SLIDING is the product (sliding 8x8 register window on even cells, groups of 4
+ * lanes with two columns per lane, k_grid_pair8.cu); PAIR7 (7x7 window moving every cell,
+ * k_grid_pair.cu) and SLIDING7 (groups of 7 lanes, one column per lane, k_grid_sliding.cu) are its
+ * predecessors, kept for comparison; ATOMIC (one thread per sample, 98 global float atomics) is the
+ * ncu comparison point the design replaces.  All four give the same image within the parity bars. */
 enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1, TOI_GRIDDER_SLIDING7 = 2, TOI_GRIDDER_PAIR7 = 3 };
 
 /* The paper's inputs (Measurement Set, image size, cell size) plus the knobs the
