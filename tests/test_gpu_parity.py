@@ -282,6 +282,28 @@ def test_edge_non_default_grid_size():
     _assert_image(img, img_o, "G=384")
 
 
+@pytest.mark.parametrize("gridder", ALL_GRIDDERS)
+@pytest.mark.parametrize("G", [198, 202, 136])
+def test_edge_grid_half_size_odd_or_tight(G, gridder):
+    """G/2 odd (198, 202): the even-aligned 8x8 register window of the product gridder then starts
+    one column/row OUTSIDE the grid for samples on the lowest on-grid cells and overhangs into the
+    plan's guard band; G = 136 barely holds the image (G >= N) so many samples sit on the edge
+    cells or fall off.  Full protocol (indices, counts, pre-FFT grid, image) for every gridder."""
+    wl = synth.reduced(synth.CONFIG1, n_ant=12, n_core=12, n_chan=48, image_size=128, cell_arcsec=25.0)
+    snap = snapshot_np(wl)
+    rc, img_o, info_o, ex = _oracle(snap, wl.image_size, wl.cell_size_deg, G=G, want_grid=True)
+    assert rc == 0 and info_o["n_gridded"] > 0
+    if G == 136:
+        assert info_o["n_off_grid"] > 0
+    with GpuImager(snap, wl.image_size, wl.cell_size_deg, "natural", gridder, grid_size=G) as gi:
+        toi.toi_debug_keep_grid(gi.plan, True)
+        img, info, _ = gi.image()
+        grid = gi.grid_centred()
+    assert info["n_gridded"] == info_o["n_gridded"] and info["n_off_grid"] == info_o["n_off_grid"]
+    assert rel_l2(grid.view(np.float32).ravel(), ex["grid"].view(np.float64).ravel()) <= 3e-6
+    _assert_image(img, img_o, "G=%d" % G)
+
+
 def test_no_jacobian_option():
     wl = synth.reduced(synth.CONFIG5, n_ant=12, n_core=9, n_chan=64, image_size=128)
     snap = snapshot_np(wl)
