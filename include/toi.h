@@ -191,6 +191,35 @@ int toi_image_stream(toi_plan *plan, int64_t n_snapshots, toi_fill_fn fill, void
                      toi_sink_fn sink, void *sink_user, int32_t want_info, toi_stream_stats *stats);
 
 /*
+ * Near-coplanar ("3-D") mode, PAPER.md:202-269 (section 3.4, Eqs. 17-27): the residual coordinate
+ * r3 = rho3 s_c (third row of R = B V^T) is kept.  Its range is cut into n_slab equal slabs; inside
+ * a slab the residual phase is expanded in K Chebyshev polynomials (Jacobi-Anger), so the image is
+ *   I(t1,t2) = Re{ sum_p exp(i 2 pi r3_p t3) sum_k c_k(2 pi Delta_r3 t3) M_pk(t1,t2) } / (omega Wsum)
+ * with t3(t1,t2) of Eq. 17, c_0 = J_0, c_k = 2 i^k J_k (Eq. 22) and each Chebyshev moment M_pk one
+ * gridding (samples of slab p times T_k(s_q), Eq. 19) + inverse FFT + correction/crop -- n_slab * K
+ * passes of the 2-D machinery.  Pixels outside the sphere constraint of Eq. 17 are NaN.
+ *   n_slab, K   0 = chosen from the snapshot as the paper prescribes (Eqs. 25-27: alpha_target = 10;
+ *               smallest K in {8, 16, 24, 32} whose sampled expansion error is below 1e-2), else
+ *               taken as given (1 <= n_slab <= 1024, 1 <= K <= 64)
+ *   info3       NULL or filled; info NULL or filled (counts, V, wsum; stage times are not split)
+ * This call SYNCHRONISES the stream once (the slab layout needs the snapshot's r3 range and V on
+ * the host) and allocates its three work buffers at the first call.  Readings G24-G26 of DESIGN.md.
+ * Other arguments and the returned image as toi_image_snapshot.  Needs grid_size <= 32768.
+ */
+typedef struct {
+    int32_t n_slab, K, n_passes, reserved;
+    double phi_max;             /* Eq. 26 */
+    double t3_max;              /* Eq. 25 over the image */
+    double r3_min, r3_max;      /* wavelengths */
+    double alpha_slab;          /* phi_max / n_slab */
+    double expansion_error;     /* sampled max |exp(i a s) - sum_k c_k T_k| for the K used */
+    float ms_total;
+} toi_3d_info;
+int toi_image_snapshot_3d(toi_plan *plan, const double *uvw_m, const void *vis, const float *weights,
+                          const uint8_t *flags, void *cuda_stream, int32_t n_slab, int32_t K,
+                          float **d_image_out, toi_3d_info *info3, toi_snapshot_info *info);
+
+/*
  * Re-projection ("interpolate" stage, section 3.3 Eqs. 9-16, Appendix A): resample
  * a dirty image from the tilted (t1, t2) plane it was reconstructed on to the standard (l, m) grid
  * of the same size and cell size.  GATHER: output pixel (i, j) is the direction

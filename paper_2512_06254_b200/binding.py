@@ -23,7 +23,8 @@ TOI_REPROJECT_EXACT, TOI_REPROJECT_PAPER = 0, 1
 TOI_OUT_TILTED, TOI_OUT_REPROJECT_EXACT, TOI_OUT_REPROJECT_PAPER = 0, 1, 2
 
 EXPORTS = ["toi_plan_create", "toi_plan_destroy", "toi_image_snapshot", "toi_plan_sync",
-           "toi_copy_image_to_host", "toi_image_stream", "toi_stream_set_output", "toi_reproject", "toi_difference",
+           "toi_copy_image_to_host", "toi_image_stream", "toi_stream_set_output", "toi_image_snapshot_3d",
+           "toi_reproject", "toi_difference",
            "toi_last_error", "toi_last_launch_count",
            "toi_debug_set_transform", "toi_debug_cell_indices", "toi_debug_keep_grid",
            "toi_debug_copy_grid", "toi_debug_copy_density"]
@@ -50,6 +51,15 @@ class toi_snapshot_info(C.Structure):
         d["V"] = [list(self.V[3 * r:3 * r + 3]) for r in range(3)]
         d["sing"] = list(self.sing)
         return d
+
+
+class toi_3d_info(C.Structure):
+    _fields_ = [("n_slab", C.c_int32), ("K", C.c_int32), ("n_passes", C.c_int32), ("reserved", C.c_int32),
+                ("phi_max", C.c_double), ("t3_max", C.c_double), ("r3_min", C.c_double), ("r3_max", C.c_double),
+                ("alpha_slab", C.c_double), ("expansion_error", C.c_double), ("ms_total", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
 
 
 class toi_snapshot_buffers(C.Structure):
@@ -108,6 +118,8 @@ def load(build_if_missing: bool = True):
     lib.toi_copy_image_to_host.argtypes = [vp, vp, vp]
     lib.toi_image_stream.argtypes = [vp, i64, toi_fill_fn, vp, toi_sink_fn, vp, i32, C.POINTER(toi_stream_stats)]
     lib.toi_stream_set_output.argtypes = [vp, C.POINTER(toi_stream_output)]
+    lib.toi_image_snapshot_3d.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, C.POINTER(vp), C.POINTER(toi_3d_info),
+                                          C.POINTER(toi_snapshot_info)]
     lib.toi_reproject.argtypes = [vp, vp, vp, i32, vp, vp]
     lib.toi_difference.argtypes = [vp, vp, vp, vp, vp]
     lib.toi_last_error.argtypes = [vp]
@@ -174,6 +186,19 @@ def toi_image_snapshot(plan, uvw_m, vis, weights=None, flags=None, stream=None, 
                                 C.byref(info) if want_info else None)
     _check(plan, rc, allow=(TOI_ERR_DEGENERATE_GEOMETRY,) if allow_degenerate else ())
     return out.value, info, rc
+
+
+def toi_image_snapshot_3d(plan, uvw_m, vis, weights=None, flags=None, stream=None, n_slab=0, K=0, want_info=True):
+    """Near-coplanar (3-D) mode.  -> (device image pointer int, toi_3d_info dict, toi_snapshot_info|None)."""
+    lib = load()
+    out = C.c_void_p()
+    i3 = toi_3d_info()
+    info = toi_snapshot_info() if want_info else None
+    s = None if stream is None else C.c_void_p(stream.cuda_stream)
+    rc = lib.toi_image_snapshot_3d(plan, _ptr(uvw_m), _ptr(vis), _ptr(weights), _ptr(flags), s, int(n_slab), int(K),
+                                   C.byref(out), C.byref(i3), C.byref(info) if want_info else None)
+    _check(plan, rc)
+    return out.value, i3.as_dict(), info
 
 
 def toi_plan_sync(plan, allow=()):

@@ -269,11 +269,15 @@ __device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, bo
     }
 }
 
-template <int MODE, int OPT, bool PIPE>
+// CHEB: one Chebyshev-moment pass of the near-coplanar mode (struct ChebArgs): only the samples of
+// slab cheb.p contribute, each multiplied by T_k(s_q); never combined with PIPE (the current sample's
+// channel scale is needed for r3).
+template <int MODE, int OPT, bool PIPE, bool CHEB>
 __global__ void __launch_bounds__(kWarps * 32, ctas_per_sm(PIPE))
 k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__restrict__ D,
-            float2 *__restrict__ grid, int strip_len, int tasks_per_row, unsigned n_tasks)
+            float2 *__restrict__ grid, int strip_len, int tasks_per_row, unsigned n_tasks, ChebArgs cheb)
 {
+    static_assert(!(PIPE && CHEB), "the Chebyshev pass computes the cell in place");
     __shared__ uint4 s_rec[kWarps * kWarpQuads];
     if (st->status != TOI_OK) return;
     const bool has_w = OPT >= 0 ? (OPT & kHasW) != 0 : in.weights != nullptr;
@@ -295,6 +299,7 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
 
     double wsum = 0.0;
     unsigned n_grid = 0, n_off = 0, n_flag = 0;
+    const bool count = !CHEB || cheb.count != 0;   // Chebyshev passes with k > 0 repeat the samples: count once
 
     for (;;) {
         unsigned task = 0;
@@ -305,6 +310,7 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
         const int c_task = (int)(task % (unsigned)tasks_per_row) * (kGroups * strip_len);
         double rho1, rho2;
         rotate_baseline(st->V, in.uvw + 3 * j, rho1, rho2);
+        const double rho3 = CHEB ? rotate_row3(st->V, in.uvw + 3 * j) : 0.0;
         const int c_lo = c_task + grp * strip_len + pre_k;        // my channel in batch 0
         const int c_hi = min(c_task + (grp + 1) * strip_len, g.n_c);
         const long long q_row = (long long)j * g.n_c;
@@ -329,7 +335,7 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                 cl.key = cell_key(bu, bv);
                 cl.sh = (unsigned)((iu - kH) & 1) | ((unsigned)((iv - kH) & 1) << 1);
                 if (has_d) cl.dens = __ldg(Dc + ((long long)iv * G + iu));
-            } else {
+            } else if (count) {
                 ++n_off;
             }
         };
@@ -373,14 +379,35 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                     const float wa = (weight_ok(cur.wa) && !(cur.fl & 0x000000ffu)) ? cur.wa : 0.0f;
                     const float wb = (weight_ok(cur.wb) && !(cur.fl & fmask_b)) ? cur.wb : 0.0f;
                     wI = wa + wb;
+                    float tk = 1.0f;
+                    bool mine = true;
+                    if (CHEB && wI > 0.0f) {
+                        // Eq. 19: slab of this sample and its position s_q in it (G24); T_k(s_q) by the
+                        // three-term recurrence in fp64 (T_k amplifies rounding by ~k^2)
+                        const double r3 = __dmul_rn(rho3, cur.s);
+                        int pq = 0;
+                        double sq = 0.0;
+                        if (cheb.d > 0.0) {
+                            pq = min((int)floor((r3 - cheb.r3_min) / (2.0 * cheb.d)), cheb.n_slab - 1);
+                            sq = (r3 - (cheb.r3_min + (2.0 * (double)pq + 1.0) * cheb.d)) / cheb.d;
+                        }
+                        mine = pq == cheb.p;
+                        double t0 = 1.0, t1 = sq;
+                        for (int kk = 1; kk < cheb.k; ++kk) {
+                            const double t2 = fma(2.0 * sq, t1, -t0);
+                            t0 = t1; t1 = t2;
+                        }
+                        tk = (float)(cheb.k == 0 ? 1.0 : t1);
+                    }
                     if (!(wI > 0.0f)) {
-                        ++n_flag;
-                    } else {
-                        ++n_grid;
+                        if (count) ++n_flag;
+                    } else if (mine) {
+                        if (count) ++n_grid;
                         valid = true;
                         // z = w_a Vis_a + w_b Vis_b; a zero-weight hand is skipped (its data may be NaN)
                         if (wa > 0.0f) { zx = wa * cur.a.x; zy = wa * cur.a.y; }
                         if (wb > 0.0f) { zx = fmaf(wb, cur.b.x, zx); zy = fmaf(wb, cur.b.y, zy); }
+                        if (CHEB) { zx *= tk; zy *= tk; }
                         float pu[kW], pv[kW];
                         kernel_taps2(cell.xu, cell.xv, pu, pv);
                         // the 7 taps sit at window offset 0 or 1 on each axis; the free end is zero
@@ -410,7 +437,7 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                     const float dens = valid ? cell.dens : 1.0f;
                     asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(f) : "f"(dens));
                 }
-                wpart = fmaf(f, wI, wpart);
+                if (!CHEB || (count && valid)) wpart = fmaf(f, wI, wpart);
                 my_rec[0] = make_uint4(__float_as_uint(zx * f), __float_as_uint(zy * f), key, __float_as_uint(pv0));
             }
             __syncwarp();
@@ -442,7 +469,7 @@ template <int MODE>
 void launch_mode(int opt, dim3 grid, dim3 block, cudaStream_t stream, const Geometry &g, const Inputs &in,
                  SnapState *st, const float *D, float2 *d_grid, int strip, int tasks_per_row, unsigned n_tasks)
 {
-#define TOI_LAUNCH(O, P) k_grid_pair8<MODE, O, P><<<grid, block, 0, stream>>>(g, in, st, D, d_grid, strip, tasks_per_row, n_tasks)
+#define TOI_LAUNCH(O, P) k_grid_pair8<MODE, O, P, false><<<grid, block, 0, stream>>>(g, in, st, D, d_grid, strip, tasks_per_row, n_tasks, ChebArgs())
     switch (opt) {
     case kHasW | kHasF | kHasD: TOI_LAUNCH(kHasW | kHasF | kHasD, true); break;
     case kHasW | kHasF: TOI_LAUNCH(kHasW | kHasF, false); break;
@@ -484,6 +511,30 @@ void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const
         launch_mode<2>(opt, grid, block, stream, g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks);
     else
         launch_mode<0>(-1, grid, block, stream, g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks);
+}
+
+// One Chebyshev-moment pass of the near-coplanar mode (G <= 32768; the caller checks).
+void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
+                            float2 *d_grid, int n_sms, const ChebArgs &cheb, cudaStream_t stream)
+{
+    const int kCtasPerSm = ctas_per_sm(false);
+    const long long warps = (long long)kCtasPerSm * n_sms * kWarps;
+    const long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
+    const int strip = pick_strip(g.n_c, kGroups, kBatch, want, 16, 128);
+    const int tasks_per_row = (g.n_c + kGroups * strip - 1) / (kGroups * strip);
+    const long long n_tasks = (long long)g.n_b * tasks_per_row;
+    long long ctas = (n_tasks + kWarps - 1) / kWarps;
+    if (ctas > (long long)kCtasPerSm * n_sms) ctas = (long long)kCtasPerSm * n_sms;
+    const dim3 grid((unsigned)ctas), block(kWarps * 32);
+    const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags, av = (uintptr_t)in.vis;
+#define TOI_LAUNCH_CHEB(M) k_grid_pair8<M, -1, false, true><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks, cheb)
+    if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
+        TOI_LAUNCH_CHEB(4);
+    else if (g.n_p == 2 && g.pol_a == 0 && g.pol_b == 1 && (av & 15) == 0 && (aw & 7) == 0 && (af & 1) == 0)
+        TOI_LAUNCH_CHEB(2);
+    else
+        TOI_LAUNCH_CHEB(0);
+#undef TOI_LAUNCH_CHEB
 }
 
 }  // namespace toi

@@ -52,6 +52,21 @@ __device__ __forceinline__ void rotate_baseline(const double *V, const double *u
     rho2 = __dadd_rn(__dadd_rn(__dmul_rn(V[3], u), __dmul_rn(V[4], v)), __dmul_rn(V[5], w));
 }
 
+// third row: rho3 = V3 . uvw (metres), the residual coordinate kept by the near-coplanar mode
+__device__ __forceinline__ double rotate_row3(const double *V, const double *uvw_j)
+{
+    return __dadd_rn(__dadd_rn(__dmul_rn(V[6], uvw_j[0]), __dmul_rn(V[7], uvw_j[1])), __dmul_rn(V[8], uvw_j[2]));
+}
+
+// One Chebyshev-moment pass of the near-coplanar mode (Eqs. 19-24): the gridder
+// keeps only the samples of slab p and multiplies them by T_k(s_q).
+struct ChebArgs {
+    int p, k, n_slab;
+    int count;              // 1: this pass accumulates Wsum and the sample counters (k == 0)
+    double r3_min;          // lower end of the r3 range
+    double d;               // slab half-width Delta_r3 (0: all samples share one r3)
+};
+
 // floor(y) for |y| < 2^31 without the slow F2I/I2F conversion pipe: adding 2^52 + 2^51 with
 // round-down leaves floor(y) in the low word of the sum (the ulp there is 1), and subtracting the
 // constant again is exact.  Bit-identical to (int)floor(y).
@@ -234,6 +249,15 @@ void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const
 // elements of guard band before and after the grid: k_grid_pair8's 8 x 8 window may overhang the
 // grid by one row / column (of zeros); a multiple of 32 elements keeps the grid 256-byte aligned
 inline size_t grid_guard(int G) { return ((size_t)G + 8 + 31) / 32 * 32; }
+void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
+                            float2 *d_grid, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
+void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s_min, double s_max, double *d_out,
+                     cudaStream_t stream);
+void launch_crop_complex(const Geometry &g, const float2 *d_F, const double *d_ipsi, float2 *d_M, cudaStream_t stream);
+void launch_cheb_combine(int N, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
+                         const float2 *d_M, float2 *d_acc, int first, cudaStream_t stream);
+void launch_cheb_finish(int N, double beta_rad, const SnapState *st, int apply_jacobian, const float2 *d_acc,
+                        float *d_image, cudaStream_t stream);
 void launch_correct_crop(const Geometry &g, const float2 *d_F, const double *d_ipsi, const SnapState *st,
                          int apply_jacobian, float *d_image, cudaStream_t stream);
 void launch_reproject(int N, double beta_rad, const SnapState *st, const double *d_V, int mode, const float *d_src,

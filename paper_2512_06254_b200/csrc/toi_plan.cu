@@ -6,6 +6,7 @@
 #include <string.h>
 
 #include <chrono>
+#include <cmath>
 #include <new>
 #include <vector>
 
@@ -68,6 +69,13 @@ struct toi_plan {
     float *d_products = nullptr, *d_diff[2] = {nullptr, nullptr}, *h_out[2] = {nullptr, nullptr};
     cudaStream_t s_d2h = nullptr;
     cudaEvent_t ev_out_ready[2] = {}, ev_d2h_start[2] = {}, ev_d2h_done[2] = {}, ev_tail = nullptr;
+
+    // near-coplanar (3-D) mode: own grid (with guard band), one complex moment, complex accumulator,
+    // r3 range on the device and in pinned host memory; allocated at the first toi_image_snapshot_3d
+    float2 *d_grid3_alloc = nullptr, *d_grid3 = nullptr, *d_moment = nullptr, *d_acc3 = nullptr;
+    double *d_r3 = nullptr, *h_r3 = nullptr;
+    double s_min = 0, s_max = 0;
+    cudaEvent_t ev3_a = nullptr, ev3_b = nullptr;
 
     int deferred = TOI_OK;
     int last_launches = 0;
@@ -184,6 +192,10 @@ int free_plan(toi_plan *p)
     }
     if (p->ev_tail) cudaEventDestroy(p->ev_tail);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
+    cudaFree(p->d_grid3_alloc); cudaFree(p->d_moment); cudaFree(p->d_acc3); cudaFree(p->d_r3);
+    cudaFreeHost(p->h_r3);
+    if (p->ev3_a) cudaEventDestroy(p->ev3_a);
+    if (p->ev3_b) cudaEventDestroy(p->ev3_b);
     cudaFree(p->d_grid_keep); cudaFree(p->d_images);
     if (p->s_compute) cudaStreamDestroy(p->s_compute);
     if (p->s_copy) cudaStreamDestroy(p->s_copy);
@@ -405,6 +417,11 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     }
     p->S1 = (double)s1;
     p->S2 = (double)s2;
+    p->s_min = p->s_max = s[0];
+    for (int c = 1; c < cfg->n_channels; ++c) {
+        if (s[c] < p->s_min) p->s_min = s[c];
+        if (s[c] > p->s_max) p->s_max = s[c];
+    }
     Geometry &g = p->geo;
     g.n_b = cfg->n_baselines; g.n_c = cfg->n_channels; g.n_p = cfg->n_pols;
     g.pol_a = cfg->pol_a; g.pol_b = cfg->pol_b;
@@ -518,6 +535,221 @@ int toi_image_snapshot(toi_plan *p, const double *uvw_m, const void *vis, const 
     int rc = enqueue_imaging(p, in, stream, d_image_out);
     if (rc) return rc;
     if (info) return read_info(p, stream, info, host);
+    return TOI_OK;
+}
+
+// ---- near-coplanar (3-D) mode: host-side parameter selection (Eqs. 25-27) ----
+namespace {
+
+// Eq. 17 at (t1, t2); NaN outside the sphere constraint
+double t3_host(const double *V, double t1, double t2)
+{
+    const double a = t1 + V[2], b = t2 + V[5], rad = 1.0 - a * a - b * b;
+    if (!(rad >= 0.0)) return NAN;
+    return -V[8] + (V[8] < 0.0 ? -sqrt(rad) : sqrt(rad));
+}
+
+// Eq. 25 over the pixels of the N x N image: |t3| is extremal on the border of the image or at the
+// pixels around the stationary point (t1, t2) = (-V13, -V23) of the square root
+double t3_max_host(const double *V, int N, double beta)
+{
+    double best = 0.0;
+    auto look = [&](int i, int j) {
+        if (i < 0 || j < 0 || i >= N || j >= N) return;
+        const double t3 = t3_host(V, -beta * (double)(i - N / 2), beta * (double)(j - N / 2));
+        if (t3 == t3 && fabs(t3) > best) best = fabs(t3);
+    };
+    for (int k = 0; k < N; ++k) { look(k, 0); look(k, N - 1); look(0, k); look(N - 1, k); }
+    const int ic = (int)floor(N / 2 + V[2] / beta), jc = (int)floor(N / 2 - V[5] / beta);
+    for (int dj = -1; dj <= 2; ++dj)
+        for (int di = -1; di <= 2; ++di) look(ic + di, jc + dj);
+    // a border that leaves the sphere constraint: scan everything (small or all-sky images only)
+    bool nan_border = false;
+    for (int k = 0; k < N && !nan_border; ++k) {
+        const double a = t3_host(V, -beta * (double)(k - N / 2), beta * (double)(0 - N / 2));
+        const double b = t3_host(V, -beta * (double)(k - N / 2), beta * (double)(N - 1 - N / 2));
+        const double c = t3_host(V, -beta * (double)(0 - N / 2), beta * (double)(k - N / 2));
+        const double d = t3_host(V, -beta * (double)(N - 1 - N / 2), beta * (double)(k - N / 2));
+        nan_border = !(a == a && b == b && c == c && d == d);
+    }
+    if (nan_border)
+        for (int j = 0; j < N; ++j)
+            for (int i = 0; i < N; ++i) look(i, j);
+    return best;
+}
+
+// max over a 129 x 257 grid of [0, alpha_slab] x [-1, 1] of |exp(i a s) - sum_{k<K} c_k(a) T_k(s)| (G25)
+double sampled_error_host(double alpha_slab, int K)
+{
+    const int na = 129, ns = 257;
+    double worst = 0.0;
+    std::vector<double> J(K), T(K);
+    for (int ia = 0; ia < na; ++ia) {
+        const double a = alpha_slab * ia / (na - 1);
+        for (int k = 0; k < K; ++k) J[k] = std::cyl_bessel_j((double)k, a);
+        for (int is = 0; is < ns; ++is) {
+            const double sq = -1.0 + 2.0 * is / (ns - 1);
+            T[0] = 1.0;
+            if (K > 1) T[1] = sq;
+            for (int k = 2; k < K; ++k) T[k] = 2.0 * sq * T[k - 1] - T[k - 2];
+            double re = J[0], im = 0.0;                  // c_0 = J_0, c_k = 2 i^k J_k
+            for (int k = 1; k < K; ++k) {
+                const double v = 2.0 * J[k] * T[k];
+                switch (k & 3) { case 0: re += v; break; case 1: im += v; break; case 2: re -= v; break; default: im -= v; break; }
+            }
+            const double er = cos(a * sq) - re, ei = sin(a * sq) - im;
+            const double e = sqrt(er * er + ei * ei);
+            if (e > worst) worst = e;
+        }
+    }
+    return worst;
+}
+
+}  // namespace
+
+int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, const float *weights, const uint8_t *flags,
+                          void *cuda_stream, int32_t n_slab_in, int32_t K_in, float **d_image_out, toi_3d_info *info3,
+                          toi_snapshot_info *info)
+{
+    if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
+    if (!uvw_m || !vis || !d_image_out) return fail(p, TOI_ERR_INVALID_ARG, "uvw_m, vis and d_image_out must be non-NULL");
+    if (n_slab_in < 0 || n_slab_in > 1024 || K_in < 0 || K_in > 64) return fail(p, TOI_ERR_INVALID_ARG, "n_slab must be in [0, 1024], K in [0, 64]");
+    const Geometry &g = p->geo;
+    if (g.G > 32768) return fail(p, TOI_ERR_UNSUPPORTED, "the 3-D mode needs grid_size <= 32768");
+    CU_TRY(p, cudaSetDevice(p->cfg.device));
+    cudaStream_t stream = cuda_stream ? (cudaStream_t)cuda_stream : p->s_compute;
+    const size_t GG = (size_t)g.G * g.G, NN = (size_t)g.N * g.N;
+    if (!p->d_grid3_alloc) {
+        CU_TRY(p, cudaMalloc(&p->d_grid3_alloc, (GG + 2 * grid_guard(g.G)) * sizeof(float2)));
+        p->d_grid3 = p->d_grid3_alloc + grid_guard(g.G);
+        CU_TRY(p, cudaMalloc(&p->d_moment, NN * sizeof(float2)));
+        CU_TRY(p, cudaMalloc(&p->d_acc3, NN * sizeof(float2)));
+        CU_TRY(p, cudaMalloc(&p->d_r3, 2 * sizeof(double)));
+        CU_TRY(p, cudaMallocHost(&p->h_r3, 2 * sizeof(double)));
+        CU_TRY(p, cudaEventCreate(&p->ev3_a));
+        CU_TRY(p, cudaEventCreate(&p->ev3_b));
+    }
+    if (p->fft_stream != stream) {
+        if (cufftSetStream(p->fft, stream) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
+        if (p->fft_pruned && (cufftSetStream(p->fft_cols, stream) != CUFFT_SUCCESS ||
+                              cufftSetStream(p->fft_rows, stream) != CUFFT_SUCCESS))
+            return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
+        p->fft_stream = stream;
+    }
+    CU_TRY(p, cudaEventRecord(p->ev3_a, stream));
+    Inputs in;
+    if (p->cfg.input_location == TOI_MEM_HOST) {
+        p->snap_slot ^= 1;
+        int rc = h2d_slot(p, p->snap_slot, uvw_m, vis, weights, flags, stream, in);
+        if (rc) return rc;
+    } else {
+        in.uvw = uvw_m; in.vis = (const float2 *)vis; in.weights = weights; in.flags = flags;
+    }
+    // plane fit, r3 range -> host (the one synchronisation of this mode)
+    launch_planefit(g, in.uvw, p->S1, p->S2, p->inject ? p->d_V_inject : nullptr, p->d_state, stream);
+    launch_r3_range(g.n_b, in.uvw, p->d_state, p->s_min, p->s_max, p->d_r3, stream);
+    CU_TRY(p, cudaMemcpyAsync(p->h_state, p->d_state, sizeof(SnapState), cudaMemcpyDeviceToHost, stream));
+    CU_TRY(p, cudaMemcpyAsync(p->h_r3, p->d_r3, 2 * sizeof(double), cudaMemcpyDeviceToHost, stream));
+    CU_TRY(p, cudaStreamSynchronize(stream));
+    float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * NN;
+    ++p->ring_pos;
+    *d_image_out = img;
+    p->last_in = in;
+    if (p->h_state->status != TOI_OK) {
+        CU_TRY(p, cudaMemsetAsync(img, 0, NN * sizeof(float), stream));
+        return fail(p, p->h_state->status, "degenerate geometry: the snapshot's baselines do not span a plane (or V33 < 1e-6)");
+    }
+    const double beta = p->cfg.cell_size_deg * (3.14159265358979323846 / 180.0);
+    const double r3_min = p->h_r3[0], r3_max = p->h_r3[1];
+    const double t3_max = t3_max_host(p->h_state->V, g.N, beta);
+    const double phi_max = 2.0 * 3.14159265358979323846 * t3_max * (r3_max - r3_min) / 2.0;       // Eq. 26
+    const int n_slab = n_slab_in > 0 ? n_slab_in : (int)fmax(1.0, ceil(phi_max / 10.0));          // Eq. 27
+    if (n_slab > 1024) return fail(p, TOI_ERR_UNSUPPORTED, "more than 1024 slabs: the snapshot is far from coplanar");
+    const double alpha_slab = phi_max / n_slab;
+    int K = K_in;
+    double err = -1.0;
+    if (K == 0) {
+        const int choices[4] = {8, 16, 24, 32};
+        K = 32;
+        for (int c = 0; c < 4; ++c) {
+            const double e = sampled_error_host(alpha_slab, choices[c]);
+            if (e < 1e-2) { K = choices[c]; err = e; break; }
+        }
+    }
+    if (err < 0.0 && info3) err = sampled_error_host(alpha_slab, K);
+    const double d = (r3_max - r3_min) / (2.0 * n_slab);                                           // G24
+    const int slabs_run = d > 0.0 ? n_slab : 1;
+    int launches = 2;
+    // uniform weighting: the density map does not depend on the slab or the order
+    const bool uniform = p->cfg.weighting == TOI_WEIGHT_UNIFORM;
+    const float *dens = nullptr;
+    if (uniform) {
+        CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_zeroed[0], 0));
+        CU_TRY(p, cudaMemsetAsync(p->d_dens[0], 0, GG * sizeof(float), stream));
+        launch_density(g, in, p->d_state, p->d_dens[0], stream);
+        dens = p->d_dens[0];
+        launches += 2;
+    }
+    cufftComplex *F = (cufftComplex *)p->d_grid3;
+    bool first = true;
+    for (int sp = 0; sp < slabs_run; ++sp) {
+        for (int k = 0; k < K; ++k) {
+            ChebArgs ca;
+            ca.p = sp; ca.k = k; ca.n_slab = n_slab; ca.count = k == 0; ca.r3_min = r3_min; ca.d = d;
+            CU_TRY(p, cudaMemsetAsync(p->d_grid3, 0, GG * sizeof(float2), stream));
+            CU_TRY(p, cudaMemsetAsync(&p->d_state->task_counter, 0, sizeof(unsigned int), stream));
+            launch_grid_pair8_cheb(g, in, p->d_state, dens, p->d_grid3, p->n_sms, ca, stream);
+            if (p->fft_pruned) {
+                cufftComplex *Fhi = F + (g.G - g.N / 2);
+                if (cufftExecC2C(p->fft_rows, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
+                    cufftExecC2C(p->fft_cols, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
+                    cufftExecC2C(p->fft_cols, Fhi, Fhi, CUFFT_INVERSE) != CUFFT_SUCCESS)
+                    return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
+                launches += 3;
+            } else {
+                if (cufftExecC2C(p->fft, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
+                ++launches;
+            }
+            launch_crop_complex(g, p->d_grid3, p->d_ipsi, p->d_moment, stream);
+            const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
+            launch_cheb_combine(g.N, beta, p->d_state, k, r3_p, d, p->d_moment, p->d_acc3, first ? 1 : 0, stream);
+            first = false;
+            launches += 5;
+        }
+    }
+    launch_cheb_finish(g.N, beta, p->d_state, p->apply_jacobian, p->d_acc3, img, stream);
+    ++launches;
+    if (uniform) {
+        // hand the density buffer back zero-filled, as the 2-D path expects to find it
+        CU_TRY(p, cudaMemsetAsync(p->d_dens[0], 0, GG * sizeof(float), stream));
+        CU_TRY(p, cudaEventRecord(p->ev_zeroed[0], stream));
+    }
+    CU_TRY(p, cudaEventRecord(p->ev3_b, stream));
+    CU_TRY(p, cudaGetLastError());
+    p->last_launches = launches;
+    if (info3 || info) {
+        CU_TRY(p, cudaMemcpyAsync(p->h_state, p->d_state, sizeof(SnapState), cudaMemcpyDeviceToHost, stream));
+        CU_TRY(p, cudaStreamSynchronize(stream));
+    }
+    if (info3) {
+        memset(info3, 0, sizeof *info3);
+        info3->n_slab = n_slab; info3->K = K; info3->n_passes = slabs_run * K;
+        info3->phi_max = phi_max; info3->t3_max = t3_max; info3->r3_min = r3_min; info3->r3_max = r3_max;
+        info3->alpha_slab = alpha_slab; info3->expansion_error = err;
+        cudaEventElapsedTime(&info3->ms_total, p->ev3_a, p->ev3_b);
+    }
+    if (info) {
+        memset(info, 0, sizeof *info);
+        const SnapState &st = *p->h_state;
+        memcpy(info->V, st.V, sizeof st.V);
+        info->omega = st.omega;
+        memcpy(info->sing, st.sing, sizeof st.sing);
+        info->wsum = st.wsum;
+        info->n_gridded = (int64_t)st.n_gridded;
+        info->n_off_grid = (int64_t)st.n_off_grid;
+        info->n_flagged = (int64_t)st.n_flagged;
+        cudaEventElapsedTime(&info->ms_total, p->ev3_a, p->ev3_b);
+    }
     return TOI_OK;
 }
 
