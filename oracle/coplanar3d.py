@@ -6,9 +6,9 @@ into slabs, and inside a slab the residual phase exp(i alpha s_q) is expanded in
 polynomials (Jacobi-Anger), so that the image is a sum of N_slab * K two-dimensional
 reconstructions ("Chebyshev moments").
 
-Status: ORACLE ONLY.  No CUDA path exists for this mode yet (NEXT-2); this
-module and its pins are the first step of that row, written before any kernel.  Only ``tests/``
-may import it; it shares no code with the CUDA path.
+Written and pinned before the CUDA path of this mode (``toi_image_snapshot_3d``), which is checked
+against it in ``tests/test_gpu_coplanar3d.py``.  Only ``tests/`` may import it; it shares no code
+with the CUDA path.
 
 Everything here is brute force (direct Fourier sums, no gridding, no FFT) and follows the paper's
 order and notation: it is the definition the future gridded/FFT path must reach.

@@ -1,6 +1,5 @@
 """Pins of oracle/coplanar3d.py (CPU only): the near-coplanar 3-D mode of PAPER.md:202-269
-(section 3.4, Eqs. 17-27).  ORACLE ONLY -- no CUDA path exists for this mode yet (DESIGN.md
-section 9, NEXT-2).  Pins: the paper's own worked numbers (Table 1, tests/golden/), the sphere
+(section 3.4, Eqs. 17-27).  Pins: the paper's own worked numbers (Table 1, tests/golden/), the sphere
 constraint, the Jacobi-Anger identity against direct evaluation, and Eq. 23 against Eq. 18."""
 from __future__ import annotations
 
