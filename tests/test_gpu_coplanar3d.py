@@ -166,3 +166,29 @@ def test_3d_mode_uniform_weighting_and_back_to_back_calls():
             assert abs(info["wsum"] - imgs[0][2]["wsum"]) <= 2e-6 * imgs[0][2]["wsum"]
     finally:
         toi.toi_plan_destroy(plan)
+
+
+def test_3d_mode_with_host_inputs_equals_device_inputs_and_refuses_bad_arguments():
+    import ctypes as C
+    snap = make_snapshot(seed=9, flags=True)
+    N, cell = 64, 200.0 / 3600.0
+    img_dev, i3_dev, info_dev, _ = run_gpu(snap, N, cell, 2, 8)
+    n_b, n_c, n_p = snap["vis"].shape
+    plan = toi.toi_plan_create(n_b, n_c, n_p, snap["chan_freq_hz"], N, cell, input_location=toi.TOI_MEM_HOST)
+    try:
+        t = {k: (None if snap[k] is None else torch.from_numpy(np.ascontiguousarray(snap[k])).pin_memory())
+             for k in ("uvw_m", "vis", "weights", "flags")}
+        ptr, i3, info = toi.toi_image_snapshot_3d(plan, t["uvw_m"], t["vis"], t["weights"], t["flags"], n_slab=2, K=8)
+        img = toi.toi_copy_image_to_host(plan, ptr, N).numpy()
+        assert np.array_equal(np.isnan(img), np.isnan(img_dev))
+        ok = ~np.isnan(img)
+        assert np.max(np.abs(img[ok] - img_dev[ok])) <= 1e-6 * float(np.max(np.abs(img_dev[ok])))
+        assert info.n_gridded == info_dev["n_gridded"]
+        lib = toi.load()
+        out = C.c_void_p()
+        args = (C.c_void_p(t["uvw_m"].data_ptr()), C.c_void_p(t["vis"].data_ptr()), None, None, None)
+        assert lib.toi_image_snapshot_3d(plan, *args, 2000, 8, C.byref(out), None, None) == toi.TOI_ERR_INVALID_ARG
+        assert lib.toi_image_snapshot_3d(plan, *args, 1, 65, C.byref(out), None, None) == toi.TOI_ERR_INVALID_ARG
+        assert lib.toi_image_snapshot_3d(plan, None, args[1], None, None, None, 1, 8, C.byref(out), None, None) == toi.TOI_ERR_INVALID_ARG
+    finally:
+        toi.toi_plan_destroy(plan)
