@@ -65,9 +65,47 @@ __device__ __forceinline__ double t3_pixel(const double *V, int N, double beta_r
     return -V[8] + (V[8] < 0.0 ? -sqrt(rad) : sqrt(rad));
 }
 
+// J_k on a uniform grid of n_tab + 1 points over [-a_max, a_max] (one extra node on each side for
+// the 4-point stencil), by the CUDA math library's jn: K x (n_tab + 3) doubles, once per snapshot.
+// The combination kernel interpolates it (4-point Lagrange: error <= (3/128) h^4 max|d4 J_k| ~ 1e-11
+// for h = 2 a_max / 4096, a_max <= ~10) instead of calling jn per pixel and pass, which costs
+// several hundred fp64 instructions (a per-pixel Miller recurrence was slower still).
+constexpr int kJTab = 4096;
+
+__global__ void __launch_bounds__(256)
+k_bessel_table(int K, double a_max, double *__restrict__ tab)
+{
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;           // 0 .. kJTab + 2
+    const int k = blockIdx.y;
+    if (m > kJTab + 2 || k >= K) return;
+    const double h = 2.0 * a_max / (double)kJTab;
+    const double x = -a_max + (double)(m - 1) * h;
+    // J_k(-x) = (-1)^k J_k(x); the centre node is x = 0 exactly, where jn(k > 1, 0) returns NaN
+    const double v = fabs(x) < 1e-300 ? (k == 0 ? 1.0 : 0.0) : jn(k, fabs(x));
+    tab[(size_t)k * (kJTab + 3) + m] = (x < 0.0 && (k & 1)) ? -v : v;
+}
+
+__device__ __forceinline__ double bessel_lookup(const double *__restrict__ row, double a_max, double inv_h, double x)
+{
+    double u = (x + a_max) * inv_h;                                 // 0 .. kJTab
+    u = fmin(fmax(u, 0.0), (double)kJTab);
+    int i = (int)u;
+    if (i > kJTab - 1) i = kJTab - 1;
+    const double f = u - (double)i;                                 // [0, 1]
+    const double *p = row + i;                                      // nodes i-1, i, i+1, i+2 (row is offset by one)
+    const double y0 = __ldg(p), y1 = __ldg(p + 1), y2 = __ldg(p + 2), y3 = __ldg(p + 3);
+    // 4-point Lagrange on nodes -1, 0, 1, 2
+    const double w0 = -f * (f - 1.0) * (f - 2.0) * (1.0 / 6.0);
+    const double w1 = (f + 1.0) * (f - 1.0) * (f - 2.0) * 0.5;
+    const double w2 = -(f + 1.0) * f * (f - 2.0) * 0.5;
+    const double w3 = (f + 1.0) * f * (f - 1.0) * (1.0 / 6.0);
+    return w0 * y0 + w1 * y1 + w2 * y2 + w3 * y3;
+}
+
 __global__ void __launch_bounds__(256)
 k_cheb_combine(int N, double beta_rad, const SnapState *__restrict__ st, int k, double r3_p, double d_r3,
-               const float2 *__restrict__ M, float2 *__restrict__ acc, int first)
+               const double *__restrict__ jrow, double a_max, const float2 *__restrict__ M, float2 *__restrict__ acc,
+               int first)
 {
     const int i = blockIdx.x * 32 + (threadIdx.x & 31);
     const int j = blockIdx.y * 8 + (threadIdx.x >> 5);
@@ -78,10 +116,11 @@ k_cheb_combine(int N, double beta_rad, const SnapState *__restrict__ st, int k, 
     if (t3 == t3) {
         const double two_pi = 6.283185307179586476925286766559;
         const double alpha = two_pi * d_r3 * t3;                         // Eq. 20
-        double ck = jn(k, alpha);                                        // Eq. 22
+        double ck = a_max > 0.0 ? bessel_lookup(jrow, a_max, (double)kJTab / (2.0 * a_max), alpha)
+                                : (k == 0 ? 1.0 : 0.0);                  // Eq. 22 (alpha = 0 everywhere)
         if (k > 0) ck *= 2.0;
         double sp, cp;
-        sincos(two_pi * r3_p * t3, &sp, &cp);
+        sincospi(2.0 * r3_p * t3, &sp, &cp);
         // w = exp(i 2 pi r3_p t3) * i^k * ck
         double wr, wi;
         switch (k & 3) {
@@ -129,11 +168,22 @@ void launch_crop_complex(const Geometry &g, const float2 *d_F, const double *d_i
     k_crop_complex<<<grid, 256, 0, stream>>>(g.N, g.G, d_F, d_ipsi, d_M);
 }
 
+size_t bessel_table_doubles(int K) { return (size_t)K * (kJTab + 3); }
+
+void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream)
+{
+    if (!(a_max > 0.0)) return;
+    dim3 grid((kJTab + 3 + 255) / 256, K);
+    k_bessel_table<<<grid, 256, 0, stream>>>(K, a_max, d_tab);
+}
+
 void launch_cheb_combine(int N, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
-                         const float2 *d_M, float2 *d_acc, int first, cudaStream_t stream)
+                         const double *d_tab, double a_max, const float2 *d_M, float2 *d_acc, int first,
+                         cudaStream_t stream)
 {
     dim3 grid((N + 31) / 32, (N + 7) / 8);
-    k_cheb_combine<<<grid, 256, 0, stream>>>(N, beta_rad, st, k, r3_p, d_r3, d_M, d_acc, first);
+    k_cheb_combine<<<grid, 256, 0, stream>>>(N, beta_rad, st, k, r3_p, d_r3, d_tab + (size_t)k * (kJTab + 3), a_max,
+                                             d_M, d_acc, first);
 }
 
 void launch_cheb_finish(int N, double beta_rad, const SnapState *st, int apply_jacobian, const float2 *d_acc,

@@ -73,7 +73,7 @@ struct toi_plan {
     // near-coplanar (3-D) mode: own grid (with guard band), one complex moment, complex accumulator,
     // r3 range on the device and in pinned host memory; allocated at the first toi_image_snapshot_3d
     float2 *d_grid3_alloc = nullptr, *d_grid3 = nullptr, *d_moment = nullptr, *d_acc3 = nullptr;
-    double *d_r3 = nullptr, *h_r3 = nullptr;
+    double *d_r3 = nullptr, *h_r3 = nullptr, *d_jtab = nullptr;
     double s_min = 0, s_max = 0;
     cudaEvent_t ev3_a = nullptr, ev3_b = nullptr;
 
@@ -192,7 +192,7 @@ int free_plan(toi_plan *p)
     }
     if (p->ev_tail) cudaEventDestroy(p->ev_tail);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
-    cudaFree(p->d_grid3_alloc); cudaFree(p->d_moment); cudaFree(p->d_acc3); cudaFree(p->d_r3);
+    cudaFree(p->d_grid3_alloc); cudaFree(p->d_moment); cudaFree(p->d_acc3); cudaFree(p->d_r3); cudaFree(p->d_jtab);
     cudaFreeHost(p->h_r3);
     if (p->ev3_a) cudaEventDestroy(p->ev3_a);
     if (p->ev3_b) cudaEventDestroy(p->ev3_b);
@@ -625,6 +625,7 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
         CU_TRY(p, cudaMalloc(&p->d_moment, NN * sizeof(float2)));
         CU_TRY(p, cudaMalloc(&p->d_acc3, NN * sizeof(float2)));
         CU_TRY(p, cudaMalloc(&p->d_r3, 2 * sizeof(double)));
+        CU_TRY(p, cudaMalloc(&p->d_jtab, bessel_table_doubles(64) * sizeof(double)));
         CU_TRY(p, cudaMallocHost(&p->h_r3, 2 * sizeof(double)));
         CU_TRY(p, cudaEventCreate(&p->ev3_a));
         CU_TRY(p, cudaEventCreate(&p->ev3_b));
@@ -690,6 +691,10 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
         dens = p->d_dens[0];
         launches += 2;
     }
+    // J_k(alpha) for every order, tabulated once over the range alpha takes in this image (Eq. 20)
+    const double a_max = d > 0.0 ? 2.0 * 3.14159265358979323846 * d * t3_max * (1.0 + 1e-9) : 0.0;
+    launch_bessel_table(K, a_max, p->d_jtab, stream);
+    ++launches;
     cufftComplex *F = (cufftComplex *)p->d_grid3;
     bool first = true;
     for (int sp = 0; sp < slabs_run; ++sp) {
@@ -712,7 +717,8 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
             }
             launch_crop_complex(g, p->d_grid3, p->d_ipsi, p->d_moment, stream);
             const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
-            launch_cheb_combine(g.N, beta, p->d_state, k, r3_p, d, p->d_moment, p->d_acc3, first ? 1 : 0, stream);
+            launch_cheb_combine(g.N, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->d_moment, p->d_acc3,
+                                first ? 1 : 0, stream);
             first = false;
             launches += 5;
         }
