@@ -8,8 +8,8 @@
 //
 //   k_r3_range      r3 range of the snapshot (Eq. 26) -- r3 = rho3 * s_c is monotone in s_c, so the
 //                   extremes sit at the band edges of the extreme baselines
-//   k_crop_complex  correction + crop of one moment, complex (k_correct_crop keeps only Re)
-//   k_cheb_combine  acc += exp(i 2 pi r3_p t3) c_k(alpha) M_pk per pixel, c_0 = J_0, c_k = 2 i^k J_k
+//   k_cheb_combine  correction + crop of one moment (complex: k_correct_crop keeps only Re) fused with
+//                   acc += exp(i 2 pi r3_p t3) c_k(alpha) M_pk per pixel, c_0 = J_0, c_k = 2 i^k J_k
 //   k_cheb_finish   image = Re(acc) / (omega Wsum); NaN outside the sphere constraint of Eq. 17
 #include <math_constants.h>
 
@@ -40,19 +40,6 @@ k_r3_range(int n_b, const double *__restrict__ uvw, const SnapState *__restrict_
         __syncthreads();
     }
     if (threadIdx.x == 0) { out[0] = s_lo[0]; out[1] = s_hi[0]; }
-}
-
-__global__ void __launch_bounds__(256)
-k_crop_complex(int N, int G, const float2 *__restrict__ F, const double *__restrict__ ipsi, float2 *__restrict__ M)
-{
-    const int i = blockIdx.x * 32 + (threadIdx.x & 31);
-    const int j = blockIdx.y * 8 + (threadIdx.x >> 5);
-    if (i >= N || j >= N) return;
-    const int n = i - (N >> 1), m = j - (N >> 1);
-    const float2 f = __ldg(F + (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n));
-    double c = ipsi[i] * ipsi[j];
-    if ((n + m) & 1) c = -c;                                 // (-1)^(n+m) of the centred grid
-    M[(size_t)j * N + i] = make_float2((float)(f.x * c), (float)(f.y * c));
 }
 
 // t3 of Eq. 17 at pixel (i, j); NaN outside the sphere constraint
@@ -103,9 +90,9 @@ __device__ __forceinline__ double bessel_lookup(const double *__restrict__ row, 
 }
 
 __global__ void __launch_bounds__(256)
-k_cheb_combine(int N, double beta_rad, const SnapState *__restrict__ st, int k, double r3_p, double d_r3,
-               const double *__restrict__ jrow, double a_max, const float2 *__restrict__ M, float2 *__restrict__ acc,
-               int first)
+k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, int k, double r3_p, double d_r3,
+               const double *__restrict__ jrow, double a_max, const float2 *__restrict__ F,
+               const double *__restrict__ ipsi, float2 *__restrict__ acc, int first)
 {
     const int i = blockIdx.x * 32 + (threadIdx.x & 31);
     const int j = blockIdx.y * 8 + (threadIdx.x >> 5);
@@ -129,10 +116,14 @@ k_cheb_combine(int N, double beta_rad, const SnapState *__restrict__ st, int k, 
         case 2: wr = -cp; wi = -sp; break;
         default: wr = sp; wi = -cp; break;
         }
-        wr *= ck; wi *= ck;
-        const float2 m = M[o];
-        a.x += (float)(wr * m.x - wi * m.y);
-        a.y += (float)(wr * m.y + wi * m.x);
+        // the moment at this pixel: cuFFT's unshifted output, (-1)^(n+m) of the centred grid, 1/(psi psi)
+        const int n = i - (N >> 1), m = j - (N >> 1);
+        const float2 f = __ldg(F + (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n));
+        double c = ipsi[i] * ipsi[j] * ck;
+        if ((n + m) & 1) c = -c;
+        wr *= c; wi *= c;
+        a.x += (float)(wr * f.x - wi * f.y);
+        a.y += (float)(wr * f.y + wi * f.x);
     }
     acc[o] = a;
 }
@@ -162,12 +153,6 @@ void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s
     k_r3_range<<<1, 256, 0, stream>>>(n_b, d_uvw, st, s_min, s_max, d_out);
 }
 
-void launch_crop_complex(const Geometry &g, const float2 *d_F, const double *d_ipsi, float2 *d_M, cudaStream_t stream)
-{
-    dim3 grid((g.N + 31) / 32, (g.N + 7) / 8);
-    k_crop_complex<<<grid, 256, 0, stream>>>(g.N, g.G, d_F, d_ipsi, d_M);
-}
-
 size_t bessel_table_doubles(int K) { return (size_t)K * (kJTab + 3); }
 
 void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream)
@@ -177,13 +162,13 @@ void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream
     k_bessel_table<<<grid, 256, 0, stream>>>(K, a_max, d_tab);
 }
 
-void launch_cheb_combine(int N, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
-                         const double *d_tab, double a_max, const float2 *d_M, float2 *d_acc, int first,
-                         cudaStream_t stream)
+void launch_cheb_combine(const Geometry &g, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
+                         const double *d_tab, double a_max, const float2 *d_F, const double *d_ipsi, float2 *d_acc,
+                         int first, cudaStream_t stream)
 {
-    dim3 grid((N + 31) / 32, (N + 7) / 8);
-    k_cheb_combine<<<grid, 256, 0, stream>>>(N, beta_rad, st, k, r3_p, d_r3, d_tab + (size_t)k * (kJTab + 3), a_max,
-                                             d_M, d_acc, first);
+    dim3 grid((g.N + 31) / 32, (g.N + 7) / 8);
+    k_cheb_combine<<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k, r3_p, d_r3, d_tab + (size_t)k * (kJTab + 3),
+                                             a_max, d_F, d_ipsi, d_acc, first);
 }
 
 void launch_cheb_finish(int N, double beta_rad, const SnapState *st, int apply_jacobian, const float2 *d_acc,

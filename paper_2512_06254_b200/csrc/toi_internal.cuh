@@ -253,12 +253,11 @@ void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, 
                             float2 *d_grid, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
 void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s_min, double s_max, double *d_out,
                      cudaStream_t stream);
-void launch_crop_complex(const Geometry &g, const float2 *d_F, const double *d_ipsi, float2 *d_M, cudaStream_t stream);
 size_t bessel_table_doubles(int K);
 void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream);
-void launch_cheb_combine(int N, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
-                         const double *d_tab, double a_max, const float2 *d_M, float2 *d_acc, int first,
-                         cudaStream_t stream);
+void launch_cheb_combine(const Geometry &g, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
+                         const double *d_tab, double a_max, const float2 *d_F, const double *d_ipsi, float2 *d_acc,
+                         int first, cudaStream_t stream);
 void launch_cheb_finish(int N, double beta_rad, const SnapState *st, int apply_jacobian, const float2 *d_acc,
                         float *d_image, cudaStream_t stream);
 void launch_correct_crop(const Geometry &g, const float2 *d_F, const double *d_ipsi, const SnapState *st,

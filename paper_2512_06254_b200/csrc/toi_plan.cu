@@ -70,9 +70,9 @@ struct toi_plan {
     cudaStream_t s_d2h = nullptr;
     cudaEvent_t ev_out_ready[2] = {}, ev_d2h_start[2] = {}, ev_d2h_done[2] = {}, ev_tail = nullptr;
 
-    // near-coplanar (3-D) mode: own grid (with guard band), one complex moment, complex accumulator,
+    // near-coplanar (3-D) mode: own grid (with guard band), complex accumulator,
     // r3 range on the device and in pinned host memory; allocated at the first toi_image_snapshot_3d
-    float2 *d_grid3_alloc = nullptr, *d_grid3 = nullptr, *d_moment = nullptr, *d_acc3 = nullptr;
+    float2 *d_grid3_alloc = nullptr, *d_grid3 = nullptr, *d_acc3 = nullptr;
     double *d_r3 = nullptr, *h_r3 = nullptr, *d_jtab = nullptr;
     double s_min = 0, s_max = 0;
     cudaEvent_t ev3_a = nullptr, ev3_b = nullptr;
@@ -192,7 +192,7 @@ int free_plan(toi_plan *p)
     }
     if (p->ev_tail) cudaEventDestroy(p->ev_tail);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
-    cudaFree(p->d_grid3_alloc); cudaFree(p->d_moment); cudaFree(p->d_acc3); cudaFree(p->d_r3); cudaFree(p->d_jtab);
+    cudaFree(p->d_grid3_alloc); cudaFree(p->d_acc3); cudaFree(p->d_r3); cudaFree(p->d_jtab);
     cudaFreeHost(p->h_r3);
     if (p->ev3_a) cudaEventDestroy(p->ev3_a);
     if (p->ev3_b) cudaEventDestroy(p->ev3_b);
@@ -622,7 +622,6 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     if (!p->d_grid3_alloc) {
         CU_TRY(p, cudaMalloc(&p->d_grid3_alloc, (GG + 2 * grid_guard(g.G)) * sizeof(float2)));
         p->d_grid3 = p->d_grid3_alloc + grid_guard(g.G);
-        CU_TRY(p, cudaMalloc(&p->d_moment, NN * sizeof(float2)));
         CU_TRY(p, cudaMalloc(&p->d_acc3, NN * sizeof(float2)));
         CU_TRY(p, cudaMalloc(&p->d_r3, 2 * sizeof(double)));
         CU_TRY(p, cudaMalloc(&p->d_jtab, bessel_table_doubles(64) * sizeof(double)));
@@ -715,12 +714,11 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
                 if (cufftExecC2C(p->fft, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
                 ++launches;
             }
-            launch_crop_complex(g, p->d_grid3, p->d_ipsi, p->d_moment, stream);
             const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
-            launch_cheb_combine(g.N, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->d_moment, p->d_acc3,
+            launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->d_grid3, p->d_ipsi, p->d_acc3,
                                 first ? 1 : 0, stream);
             first = false;
-            launches += 5;
+            launches += 4;
         }
     }
     launch_cheb_finish(g.N, beta, p->d_state, p->apply_jacobian, p->d_acc3, img, stream);
