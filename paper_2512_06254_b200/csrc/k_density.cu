@@ -36,8 +36,8 @@ k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__rest
         if (c < g.n_c) {
             s[u] = __ldg(g.s + c);
             if (FAST) {
-                if (in.weights) w4[u] = __ldg(reinterpret_cast<const float4 *>(in.weights) + (q_row + c));
-                if (in.flags) fl[u] = __ldg(reinterpret_cast<const unsigned *>(in.flags) + (q_row + c));
+                if (in.weights) w4[u] = __ldcs(reinterpret_cast<const float4 *>(in.weights) + (q_row + c));
+                if (in.flags) fl[u] = __ldcs(reinterpret_cast<const unsigned *>(in.flags) + (q_row + c));
             }
         }
     }
