@@ -458,3 +458,36 @@ def test_config2_full_size(weighting):
     assert rc == 0
     peak = float(np.max(np.abs(img_o)))
     assert np.max(np.abs(img_g[pj, pi] - re)) <= MAX_ABS_BAR * peak
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("cfg,n_dft", [(5, 8), (4, 6)])
+def test_configs_4_and_5_full_size(cfg, n_dft):
+    """BASELINE.json configs[3] (2016 x 32768 channels, 8192^2 image, G = 16384: 3.4 GB of inputs, a
+    2.1 GB grid) and configs[4] (low elevation, 1024 channels, 4096^2 image, G = 8192) at full size,
+    natural weighting, in the launch configuration bench.py times: whole image against Tier G, counts
+    and Wsum, and sampled pixels against the direct DFT of Eq. 7 (Tier D)."""
+    wl = synth.CONFIGS[cfg]
+    dev = synth.make_snapshot(wl, 0, device="cuda")
+    snap = {k: (v.cpu().numpy() if v is not None else None) for k, v in dev.items()}
+    del dev
+    torch.cuda.empty_cache()
+    N, cell = wl.image_size, wl.cell_size_deg
+    rc, img_o, info_o, _ = _oracle(snap, N, cell, "natural", pol_a=0, pol_b=3)
+    assert rc == 0
+    with GpuImager(snap, N, cell, "natural", pol_a=0, pol_b=3) as gi:
+        img_g, info_g, _ = gi.image()
+    assert np.max(np.abs(np.array(info_g["V"]) - info_o["V"])) <= 1e-12
+    for k in ("n_gridded", "n_off_grid", "n_flagged"):
+        assert abs(info_g[k] - info_o[k]) <= max(2, info_o["n_gridded"] // 100000), k    # own V on both sides (G5 iii)
+    assert abs(info_g["wsum"] - info_o["wsum"]) <= 2e-6 * abs(info_o["wsum"])
+    _assert_image(img_g, img_o, "config %d natural" % cfg)
+    rng = np.random.default_rng(cfg)
+    jj, ii = np.unravel_index(np.argmax(img_o), img_o.shape)
+    pi = np.concatenate([[N // 2, ii], rng.integers(0, N, n_dft - 2)]).astype(np.int32)
+    pj = np.concatenate([[N // 2, jj], rng.integers(0, N, n_dft - 2)]).astype(np.int32)
+    rc, re, _, _ = oracle.image_dft_pixels(snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"],
+                                           snap["chan_freq_hz"], N, cell, pi, pj, pol_a=0, pol_b=3)
+    assert rc == 0
+    peak = float(np.max(np.abs(img_o)))
+    assert np.max(np.abs(img_g[pj, pi] - re)) <= MAX_ABS_BAR * peak
