@@ -24,9 +24,9 @@ namespace {
 
 constexpr int kGroups = 8;        // 4-lane groups per warp
 constexpr int kBatch = 4;         // samples per group per pre-processing batch (8 * 4 = 32 lanes)
-constexpr int kWarps = 4;         // warps per CTA
+constexpr int kWarps = 8;         // warps per CTA
 constexpr int kR = 8;             // rows (and column slots) of the register window
-constexpr int ctas_per_sm(bool pipelined) { return pipelined ? 4 : 4; }
+constexpr int ctas_per_sm(bool) { return 2; }          // 16 warps/SM at <= 128 registers (4 x 4 warps measured 1 % slower)
 constexpr int kRecQuads = 5;      // record = 5 x 16 B: {zre, zim, wkey, pv0} {pv1..4} {pv5..7, 0} {pu0..3} {pu4..7}
 constexpr int kGroupQuads = kBatch * kRecQuads;          // 20; group g sits at quad 20 g + (g >> 1):
 constexpr int kWarpQuads = kGroups * kGroupQuads + 4;    // conflict-free STS.128 / LDS.128, spread tap words
