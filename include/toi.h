@@ -49,11 +49,11 @@ enum {
 enum { TOI_WEIGHT_NATURAL = 0, TOI_WEIGHT_UNIFORM = 1 };
 enum { TOI_MEM_HOST = 0, TOI_MEM_DEVICE = 1 };
 /* gridding kernels: SLIDING is the product (sliding 8x8 register window on even cells, groups of 4
- * lanes with two columns per lane, k_grid_pair8.cu); PAIR7 (7x7 window moving every cell,
- * k_grid_pair.cu) and SLIDING7 (groups of 7 lanes, one column per lane, k_grid_sliding.cu) are its
- * predecessors, kept for comparison; ATOMIC (one thread per sample, 98 global float atomics) is the
- * ncu comparison point the design replaces.  All four give the same image within the parity bars. */
-enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1, TOI_GRIDDER_SLIDING7 = 2, TOI_GRIDDER_PAIR7 = 3 };
+ * lanes with two columns per lane, k_grid_pair8.cu); ATOMIC (one thread per sample, 98 global
+ * float atomics, k_grid_atomic.cu) is the ncu comparison point the design replaces and a second,
+ * structurally different implementation for the parity tests.  Both give the same image within
+ * the parity bars. */
+enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1 };
 
 /* The paper's inputs (Measurement Set, image size, cell size) plus the knobs the
  * paper leaves open.  Zero selects the default of every optional field. */
@@ -66,7 +66,7 @@ typedef struct {
     int32_t image_size;         /* N, even, >= 16 */
     double cell_size_deg;       /* beta of Eq. 9, degrees */
     int32_t weighting;          /* TOI_WEIGHT_* */
-    int32_t grid_size;          /* G: 0 -> 2N; even, >= N */
+    int32_t grid_size;          /* G: 0 -> 2N; even, >= N, <= 32768 */
     int32_t kernel_support;     /* W: 0 -> 7; only 7 is built */
     int32_t apply_jacobian;     /* 0 -> 1: divide by omega (Eq. 7); 2 -> do not */
     int32_t input_location;     /* TOI_MEM_*: where toi_image_snapshot's pointers live */
@@ -74,7 +74,10 @@ typedef struct {
                                    depth-1 further snapshots */
     int32_t device;             /* CUDA ordinal */
     int32_t gridder;            /* TOI_GRIDDER_* */
-    int32_t reserved[7];        /* must be 0 */
+    int32_t enable_3d;          /* 1: also allocate what toi_image_snapshot_3d needs (N*N complex
+                                   accumulator, Bessel table, r3 range) */
+    int32_t debug_keep_grid;    /* 1: also allocate the copies toi_debug_copy_grid / _density read */
+    int32_t reserved[5];        /* must be 0 */
 } toi_config;
 
 /* Filled when `info` is passed (forces a stream synchronise). */
@@ -85,12 +88,15 @@ typedef struct {
     double wsum;                /* sum_q f_q w_I,q over gridded samples: Eq. 7's N_vis */
     int64_t n_gridded, n_off_grid, n_flagged;
     float ms_h2d, ms_planefit, ms_weight, ms_grid, ms_fft, ms_crop, ms_total;
-    float ms_zero;              /* zero fill of the next snapshot's grid (+ density) on the side
-                                   stream; it runs under this snapshot's kernels */
+    float ms_clear;             /* sparse clear of the gridding grid (+ density map): only the 32x32-cell
+                                   tiles this snapshot touched are zeroed again, after the first FFT
+                                   pass has read the grid; not included in ms_fft */
 } toi_snapshot_info;
 
-/* Allocate everything: device input slots, grid ring, image ring, density, cuFFT plan,
- * correction tables, streams and events.  *out is NULL on failure. */
+/* Allocate everything: device input slots, gridding grid, FFT workspace, tile maps, image ring,
+ * density, cuFFT plans, correction tables, streams and events (and, behind cfg.enable_3d /
+ * cfg.debug_keep_grid, the buffers of the 3-D mode / of the debug exports).  Nothing is allocated
+ * by any later call except toi_stream_set_output.  *out is NULL on failure. */
 int toi_plan_create(const toi_config *cfg, toi_plan **out);
 int toi_plan_destroy(toi_plan *plan);
 
@@ -171,7 +177,8 @@ typedef struct {
  *               call host_sink(user, idx, h_image) once it has landed -- in index order, from the
  *               thread running toi_image_stream, up to two snapshots after idx was enqueued (all
  *               before toi_image_stream returns).  h_image is valid until the callback returns.
- *               Needs image_ring_depth >= 2.  A negative return aborts the run (TOI_ERR_CALLBACK).
+ *               Needs image_ring_depth >= 3 (the slot a D2H reads is never the one the next two
+ *               snapshots write).  A negative return aborts the run (TOI_ERR_CALLBACK).
  * The device sink of toi_image_stream receives the delivered image (difference or product).
  * Everything this needs is allocated HERE, not in the loop.  NULL restores the default.
  */
@@ -203,8 +210,9 @@ int toi_image_stream(toi_plan *plan, int64_t n_snapshots, toi_fill_fn fill, void
  *               taken as given (1 <= n_slab <= 1024, 1 <= K <= 64)
  *   info3       NULL or filled; info NULL or filled (counts, V, wsum; stage times are not split)
  * This call SYNCHRONISES the stream once (the slab layout needs the snapshot's r3 range and V on
- * the host) and allocates its three work buffers at the first call.  Readings G24-G26 of DESIGN.md.
- * Other arguments and the returned image as toi_image_snapshot.  Needs grid_size <= 32768.
+ * the host).  Needs a plan created with cfg.enable_3d = 1 (TOI_ERR_UNSUPPORTED otherwise): nothing
+ * is allocated here.  Readings G24-G26 of DESIGN.md.
+ * Other arguments and the returned image as toi_image_snapshot.
  */
 typedef struct {
     int32_t n_slab, K, n_passes, reserved;
@@ -236,6 +244,7 @@ int toi_image_snapshot_3d(toi_plan *plan, const double *uvw_m, const void *vis, 
  *   V        HOST row-major 3x3, or NULL = the transform of the snapshot most recently enqueued
  *            by this plan (read on the device in stream order: enqueue on the same stream, before
  *            the next snapshot).  With NULL a degenerate snapshot gives an all-NaN image.
+ *            A non-NULL V is staged in one plan-owned device buffer: use one stream for such calls.
  *   d_out    DEVICE float32 [N][N], caller-owned, must not alias d_image
  * Enqueues one kernel on cuda_stream (NULL = the plan's compute stream); does not synchronise.
  */
@@ -264,8 +273,9 @@ int toi_debug_set_transform(toi_plan *plan, const double *V);
 int toi_debug_cell_indices(toi_plan *plan, int32_t *d_iu, int32_t *d_iv);
 /* The LAST snapshot's grid before the FFT, complex64 [G][G], signed cell (kv, ku) stored CENTRED at
  * [kv + G/2][ku + G/2] (the layout the gridder writes; the (-1)^(n+m) this gives the FFT output is
- * undone in the correction kernel); DEVICE pointer.  Only valid if debug capture was enabled
- * with toi_debug_keep_grid(plan, 1) before imaging (costs one extra G*G copy per snapshot). */
+ * undone in the correction kernel); DEVICE pointer.  Needs a plan created with cfg.debug_keep_grid = 1
+ * and capture switched on with toi_debug_keep_grid(plan, 1) before imaging (costs one extra G*G copy
+ * per snapshot, and one of the density map under uniform weighting). */
 int toi_debug_keep_grid(toi_plan *plan, int32_t on);
 int toi_debug_copy_grid(toi_plan *plan, void *d_grid_c64);
 /* Uniform-weighting density of the LAST snapshot, float32 [G][G], same index convention. */

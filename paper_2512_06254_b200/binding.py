@@ -18,7 +18,7 @@ TOI_ERR_INVALID_ARG, TOI_ERR_CUDA, TOI_ERR_CUFFT, TOI_ERR_NOMEM = -1, -2, -3, -4
 TOI_ERR_DEGENERATE_GEOMETRY, TOI_ERR_CALLBACK, TOI_ERR_UNSUPPORTED = -5, -6, -7
 TOI_WEIGHT_NATURAL, TOI_WEIGHT_UNIFORM = 0, 1
 TOI_MEM_HOST, TOI_MEM_DEVICE = 0, 1
-TOI_GRIDDER_SLIDING, TOI_GRIDDER_ATOMIC, TOI_GRIDDER_SLIDING7, TOI_GRIDDER_PAIR7 = 0, 1, 2, 3
+TOI_GRIDDER_SLIDING, TOI_GRIDDER_ATOMIC = 0, 1
 TOI_REPROJECT_EXACT, TOI_REPROJECT_PAPER = 0, 1
 TOI_OUT_TILTED, TOI_OUT_REPROJECT_EXACT, TOI_OUT_REPROJECT_PAPER = 0, 1, 2
 
@@ -36,7 +36,8 @@ class toi_config(C.Structure):
                 ("image_size", C.c_int32), ("cell_size_deg", C.c_double), ("weighting", C.c_int32),
                 ("grid_size", C.c_int32), ("kernel_support", C.c_int32), ("apply_jacobian", C.c_int32),
                 ("input_location", C.c_int32), ("image_ring_depth", C.c_int32), ("device", C.c_int32),
-                ("gridder", C.c_int32), ("reserved", C.c_int32 * 7)]
+                ("gridder", C.c_int32), ("enable_3d", C.c_int32), ("debug_keep_grid", C.c_int32),
+                ("reserved", C.c_int32 * 5)]
 
 
 class toi_snapshot_info(C.Structure):
@@ -44,7 +45,7 @@ class toi_snapshot_info(C.Structure):
                 ("wsum", C.c_double), ("n_gridded", C.c_int64), ("n_off_grid", C.c_int64),
                 ("n_flagged", C.c_int64), ("ms_h2d", C.c_float), ("ms_planefit", C.c_float),
                 ("ms_weight", C.c_float), ("ms_grid", C.c_float), ("ms_fft", C.c_float),
-                ("ms_crop", C.c_float), ("ms_total", C.c_float), ("ms_zero", C.c_float)]
+                ("ms_crop", C.c_float), ("ms_total", C.c_float), ("ms_clear", C.c_float)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_ if k not in ("V", "sing")}
@@ -151,7 +152,7 @@ def _check(plan, rc, allow=()):
 def toi_plan_create(n_baselines, n_channels, n_pols, chan_freq_hz, image_size, cell_size_deg,
                     weighting=TOI_WEIGHT_NATURAL, pol_a=None, pol_b=None, grid_size=0, kernel_support=0,
                     apply_jacobian=0, input_location=TOI_MEM_DEVICE, image_ring_depth=0, device=0,
-                    gridder=TOI_GRIDDER_SLIDING):
+                    gridder=TOI_GRIDDER_SLIDING, enable_3d=False, debug_keep_grid=False):
     """-> opaque plan handle (c_void_p).  chan_freq_hz: host float64 tensor/sequence [n_channels]."""
     lib = load()
     freq = torch.as_tensor(chan_freq_hz, dtype=torch.float64, device="cpu").contiguous()
@@ -164,6 +165,7 @@ def toi_plan_create(n_baselines, n_channels, n_pols, chan_freq_hz, image_size, c
     cfg.weighting, cfg.grid_size, cfg.kernel_support = int(weighting), int(grid_size), int(kernel_support)
     cfg.apply_jacobian, cfg.input_location = int(apply_jacobian), int(input_location)
     cfg.image_ring_depth, cfg.device, cfg.gridder = int(image_ring_depth), int(device), int(gridder)
+    cfg.enable_3d, cfg.debug_keep_grid = int(bool(enable_3d)), int(bool(debug_keep_grid))
     plan = C.c_void_p()
     rc = lib.toi_plan_create(C.byref(cfg), C.byref(plan))
     _check(None, rc)

@@ -13,9 +13,11 @@
 // column slots are live (slot = column mod 8: lane c mod 4, set (c mod 8) / 4), 8 row accumulators
 // per slot.  Per record and lane: 2 FMUL2 + 16 FFMA2.  The window may overhang the grid by one
 // row / column of zeros: the plan allocates a guard band around the grid for those flushes.
-// Everything else (pre-processing, records, opaque-predicated accumulator writes, density lookup
-// one batch ahead) is k_grid_pair.cu's.
-#include <stdlib.h>
+// Pre-processing: all 32 lanes turn 32 samples (4 consecutive channels of each of the 8 strips) into
+// 80-byte shared-memory records; raw inputs (and, with a density map, the cell and its density
+// value) are requested one batch ahead.  Accumulator writes inside the window-move blocks are
+// predicated on a predicate ptxas cannot see through (`pad == 0`), which keeps it from renaming the
+// accumulators and paying 10 MOVs per record on the fast path.
 
 #include "toi_internal.cuh"
 
@@ -275,7 +277,8 @@ __device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, bo
 template <int MODE, int OPT, bool PIPE, bool CHEB>
 __global__ void __launch_bounds__(kWarps * 32, ctas_per_sm(PIPE))
 k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__restrict__ D,
-            float2 *__restrict__ grid, int strip_len, int tasks_per_row, unsigned n_tasks, ChebArgs cheb)
+            float2 *__restrict__ grid, uint8_t *__restrict__ tiles, int strip_len, int tasks_per_row,
+            unsigned n_tasks, ChebArgs cheb)
 {
     static_assert(!(PIPE && CHEB), "the Chebyshev pass computes the cell in place");
     __shared__ uint4 s_rec[kWarps * kWarpQuads];
@@ -299,7 +302,8 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
 
     double wsum = 0.0;
     unsigned n_grid = 0, n_off = 0, n_flag = 0;
-    const bool count = !CHEB || cheb.count != 0;   // Chebyshev passes with k > 0 repeat the samples: count once
+    // Chebyshev passes repeat the samples: Wsum / n_gridded once per slab, the rejects once per snapshot
+    const bool count = !CHEB || (cheb.count & 1) != 0, count_rej = !CHEB || (cheb.count & 2) != 0;
 
     for (;;) {
         unsigned task = 0;
@@ -314,6 +318,28 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
         const int c_lo = c_task + grp * strip_len + pre_k;        // my channel in batch 0
         const int c_hi = min(c_task + (grp + 1) * strip_len, g.n_c);
         const long long q_row = (long long)j * g.n_c;
+
+        // Sparse clear (k_clear.cu): mark the tiles my strip's windows can reach.  The samples of a
+        // strip lie on a ray, monotone in channel (the plan passes `tiles` only when the channel
+        // scales are monotone), so the windows stay inside the box spanned by the strip's two end
+        // samples, widened by the 4 cells a window reaches beyond its sample's centre on either side.
+        if (tiles != nullptr) {
+            const int c_first = c_task + grp * strip_len;
+            const bool some = c_first < c_hi;
+            const double s_end = __ldg(g.s + ((L & 1) ? max(c_hi - 1, 0) : min(c_first, g.n_c - 1)));
+            const double lim = (double)G;                         // far outside the grid; also absorbs NaN
+            const double eu = fmin(fmax(-__dmul_rn(__dmul_rn(rho1, s_end), g.kappa), -lim), lim);
+            const double ev = fmin(fmax(__dmul_rn(__dmul_rn(rho2, s_end), g.kappa), -lim), lim);
+            const int iu = __double2int_rd(eu + 0.5), iv = __double2int_rd(ev + 0.5);
+            const int ju = __shfl_xor_sync(0xffffffffu, iu, 1), jv = __shfl_xor_sync(0xffffffffu, iv, 1);
+            if (some && L == 0) {
+                const int h = G >> 1, tpr = tiles_per_row(G);
+                const int x0 = max(min(iu, ju) - 4 + h, 0) / kTile, x1 = min(max(iu, ju) + 4 + h, G - 1) / kTile;
+                const int y0 = max(min(iv, jv) - 4 + h, 0) / kTile, y1 = min(max(iv, jv) + 4 + h, G - 1) / kTile;
+                for (int ty = y0; ty <= y1; ++ty)
+                    for (int tx = x0; tx <= x1; ++tx) tiles[ty * tpr + tx] = 1;
+            }
+        }
 
         // sliding-window state of my group (ckey uniform across its 4 lanes)
         u64 accA[kR], accB[kR];
@@ -335,7 +361,7 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                 cl.key = cell_key(bu, bv);
                 cl.sh = (unsigned)((iu - kH) & 1) | ((unsigned)((iv - kH) & 1) << 1);
                 if (has_d) cl.dens = __ldg(Dc + ((long long)iv * G + iu));
-            } else if (count) {
+            } else if (count_rej) {
                 ++n_off;
             }
         };
@@ -400,7 +426,7 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                         tk = (float)(cheb.k == 0 ? 1.0 : t1);
                     }
                     if (!(wI > 0.0f)) {
-                        if (count) ++n_flag;
+                        if (count_rej) ++n_flag;
                     } else if (mine) {
                         if (count) ++n_grid;
                         valid = true;
@@ -467,9 +493,10 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
 
 template <int MODE>
 void launch_mode(int opt, dim3 grid, dim3 block, cudaStream_t stream, const Geometry &g, const Inputs &in,
-                 SnapState *st, const float *D, float2 *d_grid, int strip, int tasks_per_row, unsigned n_tasks)
+                 SnapState *st, const float *D, float2 *d_grid, uint8_t *tiles, int strip, int tasks_per_row,
+                 unsigned n_tasks)
 {
-#define TOI_LAUNCH(O, P) k_grid_pair8<MODE, O, P, false><<<grid, block, 0, stream>>>(g, in, st, D, d_grid, strip, tasks_per_row, n_tasks, ChebArgs())
+#define TOI_LAUNCH(O, P) k_grid_pair8<MODE, O, P, false><<<grid, block, 0, stream>>>(g, in, st, D, d_grid, tiles, strip, tasks_per_row, n_tasks, ChebArgs())
     switch (opt) {
     case kHasW | kHasF | kHasD: TOI_LAUNCH(kHasW | kHasF | kHasD, true); break;
     case kHasW | kHasF: TOI_LAUNCH(kHasW | kHasF, false); break;
@@ -484,20 +511,16 @@ void launch_mode(int opt, dim3 grid, dim3 block, cudaStream_t stream, const Geom
 
 }  // namespace
 
+// G <= 32768 (toi_plan_create checks): a window base must fit the packed 16-bit key.
 void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                       float2 *d_grid, int n_sms, cudaStream_t stream)
+                       float2 *d_grid, uint8_t *tiles, int n_sms, cudaStream_t stream)
 {
-    if (g.G > 32768) {                       // a window base would not fit the packed 16-bit key
-        launch_grid_pair(g, in, st, d_density, d_grid, n_sms, stream);
-        return;
-    }
     // strip length (channels per group per task): 8 strips per task; aim at >= 6 tasks per resident
     // warp, within [16, 128] channels and a multiple of the 4-sample batch
     const int kCtasPerSm = ctas_per_sm(d_density != nullptr);
     const long long warps = (long long)kCtasPerSm * n_sms * kWarps;
     const long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
-    int strip = pick_strip(g.n_c, kGroups, kBatch, want, 16, 128);
-    if (const char *e = getenv("TOI_STRIP")) strip = atoi(e);   // tuning override (multiple of 4)
+    const int strip = pick_strip(g.n_c, kGroups, kBatch, want, 16, 128);
     const int tasks_per_row = (g.n_c + kGroups * strip - 1) / (kGroups * strip);
     const long long n_tasks = (long long)g.n_b * tasks_per_row;
     long long ctas = (n_tasks + kWarps - 1) / kWarps;
@@ -506,16 +529,16 @@ void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const
     const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags, av = (uintptr_t)in.vis;
     const int opt = (in.weights ? kHasW : 0) | (in.flags ? kHasF : 0) | (d_density ? kHasD : 0);
     if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
-        launch_mode<4>(opt, grid, block, stream, g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks);
+        launch_mode<4>(opt, grid, block, stream, g, in, st, d_density, d_grid, tiles, strip, tasks_per_row, (unsigned)n_tasks);
     else if (g.n_p == 2 && g.pol_a == 0 && g.pol_b == 1 && (av & 15) == 0 && (aw & 7) == 0 && (af & 1) == 0)
-        launch_mode<2>(opt, grid, block, stream, g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks);
+        launch_mode<2>(opt, grid, block, stream, g, in, st, d_density, d_grid, tiles, strip, tasks_per_row, (unsigned)n_tasks);
     else
-        launch_mode<0>(-1, grid, block, stream, g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks);
+        launch_mode<0>(-1, grid, block, stream, g, in, st, d_density, d_grid, tiles, strip, tasks_per_row, (unsigned)n_tasks);
 }
 
-// One Chebyshev-moment pass of the near-coplanar mode (G <= 32768; the caller checks).
+// One Chebyshev-moment pass of the near-coplanar mode.
 void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                            float2 *d_grid, int n_sms, const ChebArgs &cheb, cudaStream_t stream)
+                            float2 *d_grid, uint8_t *tiles, int n_sms, const ChebArgs &cheb, cudaStream_t stream)
 {
     const int kCtasPerSm = ctas_per_sm(false);
     const long long warps = (long long)kCtasPerSm * n_sms * kWarps;
@@ -527,7 +550,7 @@ void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, 
     if (ctas > (long long)kCtasPerSm * n_sms) ctas = (long long)kCtasPerSm * n_sms;
     const dim3 grid((unsigned)ctas), block(kWarps * 32);
     const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags, av = (uintptr_t)in.vis;
-#define TOI_LAUNCH_CHEB(M) k_grid_pair8<M, -1, false, true><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, strip, tasks_per_row, (unsigned)n_tasks, cheb)
+#define TOI_LAUNCH_CHEB(M) k_grid_pair8<M, -1, false, true><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, tiles, strip, tasks_per_row, (unsigned)n_tasks, cheb)
     if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
         TOI_LAUNCH_CHEB(4);
     else if (g.n_p == 2 && g.pol_a == 0 && g.pol_b == 1 && (av & 15) == 0 && (aw & 7) == 0 && (af & 1) == 0)

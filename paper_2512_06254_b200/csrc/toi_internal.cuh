@@ -14,6 +14,8 @@ constexpr int kW = 7;           // kernel support (G9)
 constexpr int kH = 3;           // (W-1)/2
 constexpr float kBetaK = 16.1f; // 2.30 * W
 constexpr int kOffGrid = INT32_MIN;
+constexpr int kTile = 32;       // side of the tiles of the sparse-clear maps, cells (k_clear.cu)
+inline __host__ __device__ int tiles_per_row(int G) { return (G + kTile - 1) / kTile; }
 
 // Device-resident per-snapshot state: written by k_planefit, accumulated by the weighting and
 // gridding kernels, read by k_correct_crop.  No host round trip between the stages.
@@ -62,7 +64,9 @@ __device__ __forceinline__ double rotate_row3(const double *V, const double *uvw
 // keeps only the samples of slab p and multiplies them by T_k(s_q).
 struct ChebArgs {
     int p, k, n_slab;
-    int count;              // 1: this pass accumulates Wsum and the sample counters (k == 0)
+    int count;              // bit 0: this pass accumulates Wsum and n_gridded (k == 0: once per slab);
+                            // bit 1: it also counts the flagged and off-grid samples (p == 0, k == 0:
+                            // once per snapshot -- every pass sees all of them)
     double r3_min;          // lower end of the r3 range
     double d;               // slab half-width Delta_r3 (0: all samples share one r3)
 };
@@ -237,20 +241,22 @@ inline int pick_strip(int n_c, int groups, int batch, long long want, int lo, in
 // ---- host-side launchers, one per translation unit -------------------------------------------
 void launch_planefit(const Geometry &g, const double *d_uvw, double S1, double S2, const double *d_V_inject,
                      SnapState *st, cudaStream_t stream);
-void launch_density(const Geometry &g, const Inputs &in, SnapState *st, float *d_density, cudaStream_t stream);
+// `tiles`: byte map of the kTile x kTile-cell tiles of the grid (resp. density map) the kernel may
+// write -- it sets the entries, launch_clear_tiles zeroes those tiles again and resets them.
+void launch_density(const Geometry &g, const Inputs &in, SnapState *st, float *d_density, uint8_t *tiles,
+                    cudaStream_t stream);
 void launch_grid_atomic(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                         float2 *d_grid, cudaStream_t stream);
-void launch_grid_sliding(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                         float2 *d_grid, int n_sms, cudaStream_t stream);
-void launch_grid_pair(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                      float2 *d_grid, int n_sms, cudaStream_t stream);
+// tiles == nullptr: the caller has marked every tile itself (channel scales not monotone)
 void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                       float2 *d_grid, int n_sms, cudaStream_t stream);
+                       float2 *d_grid, uint8_t *tiles, int n_sms, cudaStream_t stream);
 // elements of guard band before and after the grid: k_grid_pair8's 8 x 8 window may overhang the
 // grid by one row / column (of zeros); a multiple of 32 elements keeps the grid 256-byte aligned
 inline size_t grid_guard(int G) { return ((size_t)G + 8 + 31) / 32 * 32; }
 void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                            float2 *d_grid, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
+                            float2 *d_grid, uint8_t *tiles, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
+void launch_clear_tiles(float2 *d_grid, int G, uint8_t *d_map, cudaStream_t stream);
+void launch_clear_tiles(float *d_density, int G, uint8_t *d_map, cudaStream_t stream);
 void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s_min, double s_max, double *d_out,
                      cudaStream_t stream);
 size_t bessel_table_doubles(int K);

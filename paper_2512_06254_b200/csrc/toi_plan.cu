@@ -41,18 +41,23 @@ struct toi_plan {
     SnapState *d_state = nullptr, *h_state = nullptr;
     DevSlot dev_in[2];
     toi_snapshot_buffers pin[2] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
-    // grid / density rings of depth 2: while snapshot n is imaged on buffer n & 1, the other buffer
-    // is zero-filled on s_zero for snapshot n + 1 (the fill is DRAM-write bound, the kernels it
-    // runs under are issue bound)
-    float2 *d_grids[2] = {nullptr, nullptr}, *d_grid_keep = nullptr;
-    float2 *d_grid_alloc[2] = {nullptr, nullptr};     // d_grids[k] = d_grid_alloc[k] + grid_guard(G)
-    float *d_dens[2] = {nullptr, nullptr};
-    cudaStream_t s_zero = nullptr;
-    cudaEvent_t ev_zeroed[2] = {}, ev_free[2] = {}, ev_z0 = nullptr, ev_z1 = nullptr;
-    int last_k = 0;
+    // ONE gridding grid (with guard band) and ONE density map, both zero between snapshots: the
+    // gridder / density pass mark the 32x32-cell tiles they write in a byte map and, once the first
+    // FFT pass has read the grid OUT OF PLACE into d_work, only those tiles are zeroed again
+    // (k_clear.cu).  The rest of the transform and the crop run on d_work.
+    float2 *d_grid = nullptr, *d_grid_alloc = nullptr;   // d_grid = d_grid_alloc + grid_guard(G)
+    float2 *d_work = nullptr;                            // FFT workspace, G x G
+    float *d_dens = nullptr;
+    uint8_t *d_tiles_grid = nullptr, *d_tiles_dens = nullptr;
+    size_t n_tiles = 0;
+    bool s_monotone = true;      // channel scales monotone: the gridder can bound a strip's tiles by its ends
+    float2 *d_grid_keep = nullptr;                       // cfg.debug_keep_grid
+    float *d_dens_keep = nullptr;
+    cudaEvent_t ev_done = nullptr;                       // end of the last imaging call (any stream)
+    cudaEvent_t ev_clear0 = nullptr, ev_clear1 = nullptr;
     float *d_images = nullptr;
     int ring_depth = 5;
-    long long ring_pos = 0;
+    long long ring_pos = 0;                              // image ring only
     bool inject = false, keep_grid = false;
     int snap_slot = 0;
     Inputs last_in = {nullptr, nullptr, nullptr, nullptr};
@@ -70,9 +75,9 @@ struct toi_plan {
     cudaStream_t s_d2h = nullptr;
     cudaEvent_t ev_out_ready[2] = {}, ev_d2h_start[2] = {}, ev_d2h_done[2] = {}, ev_tail = nullptr;
 
-    // near-coplanar (3-D) mode: own grid (with guard band), complex accumulator,
-    // r3 range on the device and in pinned host memory; allocated at the first toi_image_snapshot_3d
-    float2 *d_grid3_alloc = nullptr, *d_grid3 = nullptr, *d_acc3 = nullptr;
+    // near-coplanar (3-D) mode (cfg.enable_3d): complex accumulator, r3 range on the device and in
+    // pinned host memory, Bessel table; the passes run on d_grid / d_work like the 2-D path
+    float2 *d_acc3 = nullptr;
     double *d_r3 = nullptr, *h_r3 = nullptr, *d_jtab = nullptr;
     double s_min = 0, s_max = 0;
     cudaEvent_t ev3_a = nullptr, ev3_b = nullptr;
@@ -172,15 +177,12 @@ int free_plan(toi_plan *p)
     if (p->ev_first) cudaEventDestroy(p->ev_first);
     for (int k = 0; k < EV_COUNT; ++k)
         if (p->ev[k]) cudaEventDestroy(p->ev[k]);
-    if (p->s_zero) cudaStreamSynchronize(p->s_zero);
-    for (int k = 0; k < 2; ++k) {
-        cudaFree(p->d_grid_alloc[k]); cudaFree(p->d_dens[k]);
-        if (p->ev_zeroed[k]) cudaEventDestroy(p->ev_zeroed[k]);
-        if (p->ev_free[k]) cudaEventDestroy(p->ev_free[k]);
-    }
-    if (p->ev_z0) cudaEventDestroy(p->ev_z0);
-    if (p->ev_z1) cudaEventDestroy(p->ev_z1);
-    if (p->s_zero) cudaStreamDestroy(p->s_zero);
+    cudaFree(p->d_grid_alloc); cudaFree(p->d_work); cudaFree(p->d_dens);
+    cudaFree(p->d_tiles_grid); cudaFree(p->d_tiles_dens);
+    cudaFree(p->d_grid_keep); cudaFree(p->d_dens_keep);
+    if (p->ev_done) cudaEventDestroy(p->ev_done);
+    if (p->ev_clear0) cudaEventDestroy(p->ev_clear0);
+    if (p->ev_clear1) cudaEventDestroy(p->ev_clear1);
     if (p->s_d2h) cudaStreamSynchronize(p->s_d2h);
     cudaFree(p->d_products);
     for (int k = 0; k < 2; ++k) {
@@ -192,15 +194,68 @@ int free_plan(toi_plan *p)
     }
     if (p->ev_tail) cudaEventDestroy(p->ev_tail);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
-    cudaFree(p->d_grid3_alloc); cudaFree(p->d_acc3); cudaFree(p->d_r3); cudaFree(p->d_jtab);
+    cudaFree(p->d_acc3); cudaFree(p->d_r3); cudaFree(p->d_jtab);
     cudaFreeHost(p->h_r3);
     if (p->ev3_a) cudaEventDestroy(p->ev3_a);
     if (p->ev3_b) cudaEventDestroy(p->ev3_b);
-    cudaFree(p->d_grid_keep); cudaFree(p->d_images);
+    cudaFree(p->d_images);
     if (p->s_compute) cudaStreamDestroy(p->s_compute);
     if (p->s_copy) cudaStreamDestroy(p->s_copy);
     cudaGetLastError();
     delete p;
+    return TOI_OK;
+}
+
+int set_fft_stream(toi_plan *p, cudaStream_t stream)
+{
+    if (p->fft_stream == stream) return TOI_OK;
+    if (p->fft_ok && cufftSetStream(p->fft, stream) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
+    if (p->fft_pruned && (cufftSetStream(p->fft_cols, stream) != CUFFT_SUCCESS ||
+                          cufftSetStream(p->fft_rows, stream) != CUFFT_SUCCESS))
+        return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
+    p->fft_stream = stream;
+    return TOI_OK;
+}
+
+// The gridder marks the tiles it writes only when the channel scales are monotone (it bounds a
+// strip by its two end samples); otherwise, and for the strawman gridder, every tile is marked here.
+uint8_t *gridder_tile_map(toi_plan *p, cudaStream_t stream, bool sliding)
+{
+    if (sliding && p->s_monotone) return p->d_tiles_grid;
+    cudaMemsetAsync(p->d_tiles_grid, 1, p->n_tiles, stream);
+    return nullptr;
+}
+
+// a6, first half + sparse clear: the first FFT pass reads the grid OUT OF PLACE into the workspace,
+// after which the tiles the gridder touched are zeroed again for the next snapshot (or pass); the
+// second FFT pass runs in place on the workspace.  Returns the number of launches through *launches.
+int transform_and_clear(toi_plan *p, cudaStream_t stream, bool clear_density, bool time_clear, int *launches)
+{
+    const Geometry &g = p->geo;
+    cufftComplex *A = (cufftComplex *)p->d_grid, *F = (cufftComplex *)p->d_work;
+    if (p->fft_pruned) {
+        // row transforms of all G rows (contiguous), then column transforms of only the N columns
+        // the crop reads (columns n = -N/2..N/2-1 live at indices [0, N/2) and [G - N/2, G))
+        if (cufftExecC2C(p->fft_rows, A, F, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
+    } else {
+        if (cufftExecC2C(p->fft, A, F, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
+    }
+    ++*launches;
+    if (time_clear) CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
+    launch_clear_tiles(p->d_grid, g.G, p->d_tiles_grid, stream);
+    ++*launches;
+    if (clear_density) {
+        launch_clear_tiles(p->d_dens, g.G, p->d_tiles_dens, stream);
+        ++*launches;
+    }
+    if (time_clear) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
+    if (p->fft_pruned) {
+        cufftComplex *Fhi = F + (g.G - g.N / 2);
+        if (cufftExecC2C(p->fft_cols, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
+            cufftExecC2C(p->fft_cols, Fhi, Fhi, CUFFT_INVERSE) != CUFFT_SUCCESS)
+            return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
+        *launches += 2;
+    }
     return TOI_OK;
 }
 
@@ -210,81 +265,47 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     const Geometry &g = p->geo;
     const size_t GG = (size_t)g.G * g.G;
     int launches = 0;
-    if (p->fft_stream != stream) {
-        if (cufftSetStream(p->fft, stream) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
-        if (p->fft_pruned && (cufftSetStream(p->fft_cols, stream) != CUFFT_SUCCESS ||
-                              cufftSetStream(p->fft_rows, stream) != CUFFT_SUCCESS))
-            return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
-        p->fft_stream = stream;
-    }
-    // buffers of this snapshot (zero-filled while the previous one was imaged) and, on s_zero, the
-    // zero fill of the other pair for the next snapshot, as soon as its last reader is done
-    const int k = (int)(p->ring_pos & 1), kn = k ^ 1;
+    int rc = set_fft_stream(p, stream);
+    if (rc) return rc;
+    // one grid, one workspace: a call on another stream waits for the previous call's last kernel
+    CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_done, 0));
     const bool uniform = p->cfg.weighting == TOI_WEIGHT_UNIFORM;
-    float2 *const grid = p->d_grids[k];
     // a1-a2: plane fit (also resets the per-snapshot accumulators)
     launch_planefit(g, in.uvw, p->S1, p->S2, p->inject ? p->d_V_inject : nullptr, p->d_state, stream);
     ++launches;
-    // this snapshot's buffers were zero-filled during the previous one; the cross-stream wait is
-    // placed after the plane fit (which touches neither) so that its latency hides under that kernel
-    CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_zeroed[k], 0));
     CU_TRY(p, cudaEventRecord(p->ev[EV_FIT], stream));
-    // zero fill of the other buffer pair for the next snapshot, on s_zero, once its last reader
-    // is done and after the plane fit (one latency-bound CTA that a saturating memset would slow)
-    CU_TRY(p, cudaStreamWaitEvent(p->s_zero, p->ev[EV_FIT], 0));
-    CU_TRY(p, cudaStreamWaitEvent(p->s_zero, p->ev_free[kn], 0));
-    CU_TRY(p, cudaEventRecord(p->ev_z0, p->s_zero));
-    if (uniform) CU_TRY(p, cudaMemsetAsync(p->d_dens[kn], 0, GG * sizeof(float), p->s_zero));
-    CU_TRY(p, cudaMemsetAsync(p->d_grids[kn], 0, GG * sizeof(float2), p->s_zero));
-    CU_TRY(p, cudaEventRecord(p->ev_z1, p->s_zero));
-    CU_TRY(p, cudaEventRecord(p->ev_zeroed[kn], p->s_zero));
-    launches += uniform ? 2 : 1;
     // a4: uniform-weighting density pass
     const float *dens = nullptr;
     if (uniform) {
-        launch_density(g, in, p->d_state, p->d_dens[k], stream);
-        dens = p->d_dens[k];
+        launch_density(g, in, p->d_state, p->d_dens, p->d_tiles_dens, stream);
+        dens = p->d_dens;
         ++launches;
     }
     CU_TRY(p, cudaEventRecord(p->ev[EV_WEIGHT], stream));
-    // a3 + a5: cell indices and gridding onto the zero-filled grid
-    if (p->cfg.gridder == TOI_GRIDDER_ATOMIC)
-        launch_grid_atomic(g, in, p->d_state, dens, grid, stream);
-    else if (p->cfg.gridder == TOI_GRIDDER_SLIDING7)
-        launch_grid_sliding(g, in, p->d_state, dens, grid, p->n_sms, stream);
-    else if (p->cfg.gridder == TOI_GRIDDER_PAIR7)
-        launch_grid_pair(g, in, p->d_state, dens, grid, p->n_sms, stream);
+    // a3 + a5: cell indices and gridding onto the zero grid
+    const bool sliding = p->cfg.gridder == TOI_GRIDDER_SLIDING;
+    uint8_t *tiles = gridder_tile_map(p, stream, sliding);
+    if (sliding)
+        launch_grid_pair8(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
     else
-        launch_grid_pair8(g, in, p->d_state, dens, grid, p->n_sms, stream);
-    ++launches;
+        launch_grid_atomic(g, in, p->d_state, dens, p->d_grid, stream);
+    launches += tiles ? 1 : 2;
     CU_TRY(p, cudaEventRecord(p->ev[EV_GRID], stream));
-    if (p->keep_grid && p->d_grid_keep)
-        CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
-    // a6: inverse C2C FFT in place
-    if (p->fft_pruned) {
-        // row transforms of all G rows (contiguous), then column transforms of only the N columns
-        // the crop reads (columns n = -N/2..N/2-1 live at indices [0, N/2) and [G - N/2, G))
-        cufftComplex *F = (cufftComplex *)grid;
-        cufftComplex *Fhi = F + (g.G - g.N / 2);
-        if (cufftExecC2C(p->fft_rows, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
-            cufftExecC2C(p->fft_cols, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
-            cufftExecC2C(p->fft_cols, Fhi, Fhi, CUFFT_INVERSE) != CUFFT_SUCCESS)
-            return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
-        launches += 3;
-    } else {
-        if (cufftExecC2C(p->fft, (cufftComplex *)grid, (cufftComplex *)grid, CUFFT_INVERSE) != CUFFT_SUCCESS)
-            return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
-        ++launches;
+    if (p->keep_grid) {
+        CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
+        if (uniform) CU_TRY(p, cudaMemcpyAsync(p->d_dens_keep, p->d_dens, GG * sizeof(float), cudaMemcpyDeviceToDevice, stream));
     }
+    // a6: inverse C2C FFT, grid -> workspace, with the sparse clear of the grid inside
+    rc = transform_and_clear(p, stream, uniform, true, &launches);
+    if (rc) return rc;
     CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
     // a7: correction + crop + normalisation into the image ring
     float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
     ++p->ring_pos;
-    launch_correct_crop(g, grid, p->d_ipsi, p->d_state, p->apply_jacobian, img, stream);
+    launch_correct_crop(g, p->d_work, p->d_ipsi, p->d_state, p->apply_jacobian, img, stream);
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
-    CU_TRY(p, cudaEventRecord(p->ev_free[k], stream));
-    p->last_k = k;
+    CU_TRY(p, cudaEventRecord(p->ev_done, stream));
     CU_TRY(p, cudaGetLastError());
     p->last_in = in;
     p->last_launches = launches;
@@ -331,10 +352,11 @@ int read_info(toi_plan *p, cudaStream_t stream, toi_snapshot_info *info, bool ha
     cudaEventElapsedTime(&info->ms_weight, p->ev[EV_FIT], p->ev[EV_WEIGHT]);
     cudaEventElapsedTime(&info->ms_grid, p->ev[EV_WEIGHT], p->ev[EV_GRID]);
     cudaEventElapsedTime(&info->ms_fft, p->ev[EV_GRID], p->ev[EV_FFT]);
+    info->ms_clear = 0.0f;
+    if (cudaEventElapsedTime(&ms, p->ev_clear0, p->ev_clear1) == cudaSuccess) info->ms_clear = ms;
+    info->ms_fft -= info->ms_clear;
     cudaEventElapsedTime(&info->ms_crop, p->ev[EV_FFT], p->ev[EV_CROP]);
     cudaEventElapsedTime(&info->ms_total, p->ev[EV_START], p->ev[EV_CROP]);
-    info->ms_zero = 0.0f;
-    if (cudaEventSynchronize(p->ev_z1) == cudaSuccess) cudaEventElapsedTime(&info->ms_zero, p->ev_z0, p->ev_z1);
     cudaGetLastError();
     if (s.status != TOI_OK)
         return fail(p, s.status, "degenerate geometry: the snapshot's baselines do not span a plane (or V33 < 1e-6)");
@@ -358,17 +380,19 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
         return fail(nullptr, TOI_ERR_INVALID_ARG, "pol_a/pol_b out of range");
     if (!cfg->chan_freq_hz) return fail(nullptr, TOI_ERR_INVALID_ARG, "chan_freq_hz is NULL");
     if (N < 16 || (N & 1)) return fail(nullptr, TOI_ERR_INVALID_ARG, "image_size must be even and >= 16");
-    if ((G & 1) || G < N || G > (1 << 16)) return fail(nullptr, TOI_ERR_INVALID_ARG, "grid_size must be even, >= image_size and <= 65536");
+    // G <= 32768: the gridder packs a window's base cell into 2 x 16 bits
+    if ((G & 1) || G < N || G > 32768) return fail(nullptr, TOI_ERR_INVALID_ARG, "grid_size must be even, >= image_size and <= 32768");
     if (!(cfg->cell_size_deg > 0.0) || !(cfg->cell_size_deg < 10.0)) return fail(nullptr, TOI_ERR_INVALID_ARG, "cell_size_deg must be in (0, 10)");
     if (W != kW) return fail(nullptr, TOI_ERR_UNSUPPORTED, "only kernel_support = 7 is built");
     if (cfg->weighting != TOI_WEIGHT_NATURAL && cfg->weighting != TOI_WEIGHT_UNIFORM) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown weighting");
     if (cfg->input_location != TOI_MEM_HOST && cfg->input_location != TOI_MEM_DEVICE) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown input_location");
-    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC && cfg->gridder != TOI_GRIDDER_SLIDING7 &&
-        cfg->gridder != TOI_GRIDDER_PAIR7)
+    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC)
         return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown gridder");
+    if ((cfg->enable_3d != 0 && cfg->enable_3d != 1) || (cfg->debug_keep_grid != 0 && cfg->debug_keep_grid != 1))
+        return fail(nullptr, TOI_ERR_INVALID_ARG, "enable_3d and debug_keep_grid must be 0 or 1");
     if (cfg->image_ring_depth < 0 || cfg->image_ring_depth > 64) return fail(nullptr, TOI_ERR_INVALID_ARG, "image_ring_depth must be in [0, 64]");
     if (cfg->apply_jacobian < 0 || cfg->apply_jacobian > 2) return fail(nullptr, TOI_ERR_INVALID_ARG, "apply_jacobian must be 0, 1 or 2");
-    for (int k = 0; k < 7; ++k)
+    for (int k = 0; k < 5; ++k)
         if (cfg->reserved[k] != 0) return fail(nullptr, TOI_ERR_INVALID_ARG, "reserved fields must be 0");
     for (int c = 0; c < cfg->n_channels; ++c)
         if (!(cfg->chan_freq_hz[c] > 0.0) || !isfinite(cfg->chan_freq_hz[c]))
@@ -418,10 +442,14 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     p->S1 = (double)s1;
     p->S2 = (double)s2;
     p->s_min = p->s_max = s[0];
+    bool up = true, down = true;
     for (int c = 1; c < cfg->n_channels; ++c) {
         if (s[c] < p->s_min) p->s_min = s[c];
         if (s[c] > p->s_max) p->s_max = s[c];
+        up = up && s[c] >= s[c - 1];
+        down = down && s[c] <= s[c - 1];
     }
+    p->s_monotone = up || down;
     Geometry &g = p->geo;
     g.n_b = cfg->n_baselines; g.n_c = cfg->n_channels; g.n_p = cfg->n_pols;
     g.pol_a = cfg->pol_a; g.pol_b = cfg->pol_b;
@@ -451,24 +479,37 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     CREATE_TRY(cudaMalloc(&p->d_state, sizeof(SnapState)));
     CREATE_TRY(cudaMemset(p->d_state, 0, sizeof(SnapState)));
     CREATE_TRY(cudaMallocHost(&p->h_state, sizeof(SnapState)));
-    // default (lowest) priority: measured, a high-priority fill slows the density pass by more than it hides
-    CREATE_TRY(cudaStreamCreateWithFlags(&p->s_zero, cudaStreamNonBlocking));
-    CREATE_TRY(cudaEventCreate(&p->ev_z0));
-    CREATE_TRY(cudaEventCreate(&p->ev_z1));
-    for (int k = 0; k < 2; ++k) {
-        // guard band on both sides: the gridder's 8 x 8 window may overhang the grid by one row or
-        // column of zero accumulators, whose flush must land in owned memory (never read)
-        CREATE_TRY(cudaMalloc(&p->d_grid_alloc[k], (GG + 2 * grid_guard(G)) * sizeof(float2)));
-        CREATE_TRY(cudaMemsetAsync(p->d_grid_alloc[k], 0, (GG + 2 * grid_guard(G)) * sizeof(float2), p->s_zero));
-        p->d_grids[k] = p->d_grid_alloc[k] + grid_guard(G);
-        if (cfg->weighting == TOI_WEIGHT_UNIFORM) {
-            CREATE_TRY(cudaMalloc(&p->d_dens[k], GG * sizeof(float)));
-            CREATE_TRY(cudaMemsetAsync(p->d_dens[k], 0, GG * sizeof(float), p->s_zero));
-        }
-        CREATE_TRY(cudaEventCreateWithFlags(&p->ev_zeroed[k], cudaEventDisableTiming));
-        CREATE_TRY(cudaEventCreateWithFlags(&p->ev_free[k], cudaEventDisableTiming));
-        CREATE_TRY(cudaEventRecord(p->ev_zeroed[k], p->s_zero));
-        CREATE_TRY(cudaEventRecord(p->ev_free[k], p->s_zero));
+    // the gridding grid with a guard band on both sides (the gridder's 8 x 8 window may overhang the
+    // grid by one row or column of zero accumulators, whose flush must land in owned memory that
+    // nothing reads), zero-filled ONCE here; the FFT workspace; the density map; the tile maps
+    CREATE_TRY(cudaMalloc(&p->d_grid_alloc, (GG + 2 * grid_guard(G)) * sizeof(float2)));
+    CREATE_TRY(cudaMemset(p->d_grid_alloc, 0, (GG + 2 * grid_guard(G)) * sizeof(float2)));
+    p->d_grid = p->d_grid_alloc + grid_guard(G);
+    CREATE_TRY(cudaMalloc(&p->d_work, GG * sizeof(float2)));
+    p->n_tiles = (size_t)tiles_per_row(G) * tiles_per_row(G);
+    CREATE_TRY(cudaMalloc(&p->d_tiles_grid, p->n_tiles));
+    CREATE_TRY(cudaMemset(p->d_tiles_grid, 0, p->n_tiles));
+    if (cfg->weighting == TOI_WEIGHT_UNIFORM) {
+        CREATE_TRY(cudaMalloc(&p->d_dens, GG * sizeof(float)));
+        CREATE_TRY(cudaMemset(p->d_dens, 0, GG * sizeof(float)));
+        CREATE_TRY(cudaMalloc(&p->d_tiles_dens, p->n_tiles));
+        CREATE_TRY(cudaMemset(p->d_tiles_dens, 0, p->n_tiles));
+    }
+    CREATE_TRY(cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming));
+    CREATE_TRY(cudaEventRecord(p->ev_done, p->s_compute));
+    CREATE_TRY(cudaEventCreate(&p->ev_clear0));
+    CREATE_TRY(cudaEventCreate(&p->ev_clear1));
+    if (cfg->debug_keep_grid) {
+        CREATE_TRY(cudaMalloc(&p->d_grid_keep, GG * sizeof(float2)));
+        if (cfg->weighting == TOI_WEIGHT_UNIFORM) CREATE_TRY(cudaMalloc(&p->d_dens_keep, GG * sizeof(float)));
+    }
+    if (cfg->enable_3d) {
+        CREATE_TRY(cudaMalloc(&p->d_acc3, (size_t)N * N * sizeof(float2)));
+        CREATE_TRY(cudaMalloc(&p->d_r3, 2 * sizeof(double)));
+        CREATE_TRY(cudaMalloc(&p->d_jtab, bessel_table_doubles(64) * sizeof(double)));
+        CREATE_TRY(cudaMallocHost(&p->h_r3, 2 * sizeof(double)));
+        CREATE_TRY(cudaEventCreate(&p->ev3_a));
+        CREATE_TRY(cudaEventCreate(&p->ev3_b));
     }
     CREATE_TRY(cudaMalloc(&p->d_images, (size_t)p->ring_depth * N * N * sizeof(float)));
     if (cfg->input_location == TOI_MEM_HOST) {
@@ -483,20 +524,12 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
             CREATE_TRY(cudaMallocHost(&p->pin[k].flags, p->n_elems));
         }
     }
-    if (cufftPlan2d(&p->fft, G, G, CUFFT_C2C) != CUFFT_SUCCESS) {
-        fail(nullptr, TOI_ERR_CUFFT, "cufftPlan2d failed");
-        free_plan(p);
-        return TOI_ERR_CUFFT;
-    }
-    p->fft_ok = true;
-    // Pruned transform (default when the crop keeps at most 3/4 of the columns): 1-D transforms of
-    // all G rows, then of only the N columns the crop reads -- cuFFT's strided column pass is the
-    // expensive one (two kernels), so skipping G - N columns saves more than a third of the FFT.
-    // The skipped columns are left row-transformed only; nothing reads them.  TOI_FFT_PRUNED=0
-    // selects the plain 2-D plan.
-    bool pruned = 4 * N <= 3 * G;
-    if (const char *e = getenv("TOI_FFT_PRUNED")) pruned = pruned && atoi(e) != 0;
-    if (pruned) {
+    // Pruned transform (when the crop keeps at most 3/4 of the columns, e.g. the default G = 2N):
+    // 1-D transforms of all G rows, then of only the N columns the crop reads -- cuFFT's strided
+    // column pass is the expensive one (two kernels), so skipping G - N columns saves more than a
+    // third of the FFT.  The skipped columns are left row-transformed only; nothing reads them.
+    // Otherwise the plain 2-D plan.
+    if (4 * N <= 3 * G) {
         int n[1] = {G};
         if (cufftPlanMany(&p->fft_cols, 1, n, n, G, 1, n, G, 1, CUFFT_C2C, N / 2) != CUFFT_SUCCESS ||
             cufftPlanMany(&p->fft_rows, 1, n, n, 1, G, n, 1, G, CUFFT_C2C, G) != CUFFT_SUCCESS) {
@@ -505,6 +538,13 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
             return TOI_ERR_CUFFT;
         }
         p->fft_pruned = true;
+    } else {
+        if (cufftPlan2d(&p->fft, G, G, CUFFT_C2C) != CUFFT_SUCCESS) {
+            fail(nullptr, TOI_ERR_CUFFT, "cufftPlan2d failed");
+            free_plan(p);
+            return TOI_ERR_CUFFT;
+        }
+        p->fft_ok = true;
     }
     CREATE_TRY(cudaDeviceSynchronize());
 #undef CREATE_TRY
@@ -614,33 +654,20 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
     if (!uvw_m || !vis || !d_image_out) return fail(p, TOI_ERR_INVALID_ARG, "uvw_m, vis and d_image_out must be non-NULL");
     if (n_slab_in < 0 || n_slab_in > 1024 || K_in < 0 || K_in > 64) return fail(p, TOI_ERR_INVALID_ARG, "n_slab must be in [0, 1024], K in [0, 64]");
+    if (!p->d_acc3) return fail(p, TOI_ERR_UNSUPPORTED, "the 3-D mode needs a plan created with enable_3d = 1");
+    if (p->cfg.gridder != TOI_GRIDDER_SLIDING) return fail(p, TOI_ERR_UNSUPPORTED, "the 3-D mode runs on the sliding gridder only");
     const Geometry &g = p->geo;
-    if (g.G > 32768) return fail(p, TOI_ERR_UNSUPPORTED, "the 3-D mode needs grid_size <= 32768");
     CU_TRY(p, cudaSetDevice(p->cfg.device));
     cudaStream_t stream = cuda_stream ? (cudaStream_t)cuda_stream : p->s_compute;
     const size_t GG = (size_t)g.G * g.G, NN = (size_t)g.N * g.N;
-    if (!p->d_grid3_alloc) {
-        CU_TRY(p, cudaMalloc(&p->d_grid3_alloc, (GG + 2 * grid_guard(g.G)) * sizeof(float2)));
-        p->d_grid3 = p->d_grid3_alloc + grid_guard(g.G);
-        CU_TRY(p, cudaMalloc(&p->d_acc3, NN * sizeof(float2)));
-        CU_TRY(p, cudaMalloc(&p->d_r3, 2 * sizeof(double)));
-        CU_TRY(p, cudaMalloc(&p->d_jtab, bessel_table_doubles(64) * sizeof(double)));
-        CU_TRY(p, cudaMallocHost(&p->h_r3, 2 * sizeof(double)));
-        CU_TRY(p, cudaEventCreate(&p->ev3_a));
-        CU_TRY(p, cudaEventCreate(&p->ev3_b));
-    }
-    if (p->fft_stream != stream) {
-        if (cufftSetStream(p->fft, stream) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
-        if (p->fft_pruned && (cufftSetStream(p->fft_cols, stream) != CUFFT_SUCCESS ||
-                              cufftSetStream(p->fft_rows, stream) != CUFFT_SUCCESS))
-            return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
-        p->fft_stream = stream;
-    }
+    int rc = set_fft_stream(p, stream);
+    if (rc) return rc;
+    CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_done, 0));
     CU_TRY(p, cudaEventRecord(p->ev3_a, stream));
     Inputs in;
     if (p->cfg.input_location == TOI_MEM_HOST) {
         p->snap_slot ^= 1;
-        int rc = h2d_slot(p, p->snap_slot, uvw_m, vis, weights, flags, stream, in);
+        rc = h2d_slot(p, p->snap_slot, uvw_m, vis, weights, flags, stream, in);
         if (rc) return rc;
     } else {
         in.uvw = uvw_m; in.vis = (const float2 *)vis; in.weights = weights; in.flags = flags;
@@ -657,6 +684,7 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     p->last_in = in;
     if (p->h_state->status != TOI_OK) {
         CU_TRY(p, cudaMemsetAsync(img, 0, NN * sizeof(float), stream));
+        CU_TRY(p, cudaEventRecord(p->ev_done, stream));
         return fail(p, p->h_state->status, "degenerate geometry: the snapshot's baselines do not span a plane (or V33 < 1e-6)");
     }
     const double beta = p->cfg.cell_size_deg * (3.14159265358979323846 / 180.0);
@@ -664,7 +692,11 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     const double t3_max = t3_max_host(p->h_state->V, g.N, beta);
     const double phi_max = 2.0 * 3.14159265358979323846 * t3_max * (r3_max - r3_min) / 2.0;       // Eq. 26
     const int n_slab = n_slab_in > 0 ? n_slab_in : (int)fmax(1.0, ceil(phi_max / 10.0));          // Eq. 27
-    if (n_slab > 1024) return fail(p, TOI_ERR_UNSUPPORTED, "more than 1024 slabs: the snapshot is far from coplanar");
+    if (n_slab > 1024) {
+        CU_TRY(p, cudaMemsetAsync(img, 0, NN * sizeof(float), stream));
+        CU_TRY(p, cudaEventRecord(p->ev_done, stream));
+        return fail(p, TOI_ERR_UNSUPPORTED, "more than 1024 slabs: the snapshot is far from coplanar");
+    }
     const double alpha_slab = phi_max / n_slab;
     int K = K_in;
     double err = -1.0;
@@ -684,51 +716,44 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     const bool uniform = p->cfg.weighting == TOI_WEIGHT_UNIFORM;
     const float *dens = nullptr;
     if (uniform) {
-        CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_zeroed[0], 0));
-        CU_TRY(p, cudaMemsetAsync(p->d_dens[0], 0, GG * sizeof(float), stream));
-        launch_density(g, in, p->d_state, p->d_dens[0], stream);
-        dens = p->d_dens[0];
-        launches += 2;
+        launch_density(g, in, p->d_state, p->d_dens, p->d_tiles_dens, stream);
+        dens = p->d_dens;
+        ++launches;
     }
     // J_k(alpha) for every order, tabulated once over the range alpha takes in this image (Eq. 20)
     const double a_max = d > 0.0 ? 2.0 * 3.14159265358979323846 * d * t3_max * (1.0 + 1e-9) : 0.0;
     launch_bessel_table(K, a_max, p->d_jtab, stream);
     ++launches;
-    cufftComplex *F = (cufftComplex *)p->d_grid3;
     bool first = true;
     for (int sp = 0; sp < slabs_run; ++sp) {
         for (int k = 0; k < K; ++k) {
             ChebArgs ca;
-            ca.p = sp; ca.k = k; ca.n_slab = n_slab; ca.count = k == 0; ca.r3_min = r3_min; ca.d = d;
-            CU_TRY(p, cudaMemsetAsync(p->d_grid3, 0, GG * sizeof(float2), stream));
+            ca.p = sp; ca.k = k; ca.n_slab = n_slab; ca.r3_min = r3_min; ca.d = d;
+            ca.count = (k == 0 ? 1 : 0) | (k == 0 && sp == 0 ? 2 : 0);
+            const bool last = sp == slabs_run - 1 && k == K - 1;
             CU_TRY(p, cudaMemsetAsync(&p->d_state->task_counter, 0, sizeof(unsigned int), stream));
-            launch_grid_pair8_cheb(g, in, p->d_state, dens, p->d_grid3, p->n_sms, ca, stream);
-            if (p->fft_pruned) {
-                cufftComplex *Fhi = F + (g.G - g.N / 2);
-                if (cufftExecC2C(p->fft_rows, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
-                    cufftExecC2C(p->fft_cols, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
-                    cufftExecC2C(p->fft_cols, Fhi, Fhi, CUFFT_INVERSE) != CUFFT_SUCCESS)
-                    return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
-                launches += 3;
-            } else {
-                if (cufftExecC2C(p->fft, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
-                ++launches;
+            uint8_t *tiles = gridder_tile_map(p, stream, true);
+            launch_grid_pair8_cheb(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, ca, stream);
+            launches += tiles ? 2 : 3;
+            if (first && p->keep_grid) {
+                CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
+                if (uniform) CU_TRY(p, cudaMemcpyAsync(p->d_dens_keep, p->d_dens, GG * sizeof(float), cudaMemcpyDeviceToDevice, stream));
             }
+            // first FFT pass out of place, sparse clear of the grid (and, after the last pass, of
+            // the density map), second FFT pass on the workspace
+            rc = transform_and_clear(p, stream, uniform && last, false, &launches);
+            if (rc) return rc;
             const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
-            launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->d_grid3, p->d_ipsi, p->d_acc3,
+            launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->d_work, p->d_ipsi, p->d_acc3,
                                 first ? 1 : 0, stream);
+            ++launches;
             first = false;
-            launches += 4;
         }
     }
     launch_cheb_finish(g.N, beta, p->d_state, p->apply_jacobian, p->d_acc3, img, stream);
     ++launches;
-    if (uniform) {
-        // hand the density buffer back zero-filled, as the 2-D path expects to find it
-        CU_TRY(p, cudaMemsetAsync(p->d_dens[0], 0, GG * sizeof(float), stream));
-        CU_TRY(p, cudaEventRecord(p->ev_zeroed[0], stream));
-    }
     CU_TRY(p, cudaEventRecord(p->ev3_b, stream));
+    CU_TRY(p, cudaEventRecord(p->ev_done, stream));
     CU_TRY(p, cudaGetLastError());
     p->last_launches = launches;
     if (info3 || info) {
@@ -794,8 +819,11 @@ int toi_stream_set_output(toi_plan *p, const toi_stream_output *out)
     for (int k = 0; k < 5; ++k)
         if (o.reserved[k] != 0) return fail(p, TOI_ERR_INVALID_ARG, "reserved fields must be 0");
     if (o.to_host && !o.host_sink) return fail(p, TOI_ERR_INVALID_ARG, "to_host needs a host_sink callback");
-    if ((o.to_host || o.difference) && p->ring_depth < 2)
-        return fail(p, TOI_ERR_INVALID_ARG, "difference / to_host need image_ring_depth >= 2");
+    if (o.difference && p->ring_depth < 2) return fail(p, TOI_ERR_INVALID_ARG, "difference needs image_ring_depth >= 2");
+    // the D2H of image n runs under the imaging of n + 1 and n + 2 (its pinned slot is reclaimed just
+    // before n + 2 is enqueued... and the copy stream may lag): the ring slot it reads must not be
+    // the one either of them writes
+    if (o.to_host && p->ring_depth < 3) return fail(p, TOI_ERR_INVALID_ARG, "to_host needs image_ring_depth >= 3");
     CU_TRY(p, cudaSetDevice(p->cfg.device));
     CU_TRY(p, cudaDeviceSynchronize());
     const size_t img_bytes = (size_t)p->geo.N * p->geo.N * sizeof(float);
@@ -853,11 +881,21 @@ int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *f
         return TOI_OK;
     };
     int64_t n = 0;
+    // inside the loop an error must not return before the streams are drained and the pending host
+    // images handed over: record it and leave the loop
+#define LOOP_TRY(expr)                                                                                \
+    {                                                                                                 \
+        cudaError_t e_ = (expr);                                                                      \
+        if (e_ != cudaSuccess) {                                                                      \
+            rc = fail(p, e_ == cudaErrorMemoryAllocation ? TOI_ERR_NOMEM : TOI_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+            break;                                                                                    \
+        }                                                                                             \
+    }
     for (; n < n_snapshots; ++n) {
         const int slot = (int)(n & 1);
         if (used[slot]) {
             // the pinned slot is free once its H2D finished; compute of n-2 is long done
-            CU_TRY(p, cudaEventSynchronize(p->ev_h2d_done[slot]));
+            LOOP_TRY(cudaEventSynchronize(p->ev_h2d_done[slot]));
             harvest(slot);
         }
         toi_snapshot_buffers b = p->pin[slot];
@@ -866,22 +904,22 @@ int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *f
         if (frc < 0) { rc = fail(p, TOI_ERR_CALLBACK, "fill callback failed"); break; }
         if (!b.uvw_m || !b.vis) { rc = fail(p, TOI_ERR_CALLBACK, "fill callback returned NULL uvw/vis"); break; }
         // device slot is free once the imaging that read it finished: GPU-side wait only
-        if (used[slot]) CU_TRY(p, cudaStreamWaitEvent(p->s_copy, p->ev_c_done[slot], 0));
-        if (n == 0) CU_TRY(p, cudaEventRecord(p->ev_first, p->s_copy));
-        CU_TRY(p, cudaEventRecord(p->ev_h2d_start[slot], p->s_copy));
+        if (used[slot]) LOOP_TRY(cudaStreamWaitEvent(p->s_copy, p->ev_c_done[slot], 0));
+        if (n == 0) LOOP_TRY(cudaEventRecord(p->ev_first, p->s_copy));
+        LOOP_TRY(cudaEventRecord(p->ev_h2d_start[slot], p->s_copy));
         Inputs in;
         rc = h2d_slot(p, slot, b.uvw_m, b.vis, b.weights, b.flags, p->s_copy, in);
         if (rc) break;
-        CU_TRY(p, cudaEventRecord(p->ev_h2d_done[slot], p->s_copy));
+        LOOP_TRY(cudaEventRecord(p->ev_h2d_done[slot], p->s_copy));
         st.h2d_bytes += (double)input_bytes(p, b.weights != nullptr, b.flags != nullptr);
-        CU_TRY(p, cudaStreamWaitEvent(p->s_compute, p->ev_h2d_done[slot], 0));
-        CU_TRY(p, cudaEventRecord(p->ev_c_start[slot], p->s_compute));
-        CU_TRY(p, cudaEventRecord(p->ev[EV_START], p->s_compute));
-        CU_TRY(p, cudaEventRecord(p->ev[EV_H2D], p->s_compute));
+        LOOP_TRY(cudaStreamWaitEvent(p->s_compute, p->ev_h2d_done[slot], 0));
+        LOOP_TRY(cudaEventRecord(p->ev_c_start[slot], p->s_compute));
+        LOOP_TRY(cudaEventRecord(p->ev[EV_START], p->s_compute));
+        LOOP_TRY(cudaEventRecord(p->ev[EV_H2D], p->s_compute));
         float *img = nullptr;
         rc = enqueue_imaging(p, in, p->s_compute, &img);
         if (rc) break;
-        CU_TRY(p, cudaEventRecord(p->ev_c_done[slot], p->s_compute));
+        LOOP_TRY(cudaEventRecord(p->ev_c_done[slot], p->s_compute));
         used[slot] = true;
         // interpolate stage: tilted plane -> (l, m) grid with this snapshot's V
         float *prod = img;
@@ -910,17 +948,17 @@ int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *f
             prev_prod = prod;
         }
         if (oc.product != TOI_OUT_TILTED || oc.difference) {
-            CU_TRY(p, cudaGetLastError());
-            CU_TRY(p, cudaEventRecord(p->ev_tail, p->s_compute));
+            LOOP_TRY(cudaGetLastError());
+            LOOP_TRY(cudaEventRecord(p->ev_tail, p->s_compute));
             tail_used = true;
         }
         if (to_host) {
             // copy_cpu stage: third stream, pinned ring, events only
-            CU_TRY(p, cudaEventRecord(p->ev_out_ready[o], p->s_compute));
-            CU_TRY(p, cudaStreamWaitEvent(p->s_d2h, p->ev_out_ready[o], 0));
-            CU_TRY(p, cudaEventRecord(p->ev_d2h_start[o], p->s_d2h));
-            CU_TRY(p, cudaMemcpyAsync(p->h_out[o], deliver, n_pix * sizeof(float), cudaMemcpyDeviceToHost, p->s_d2h));
-            CU_TRY(p, cudaEventRecord(p->ev_d2h_done[o], p->s_d2h));
+            LOOP_TRY(cudaEventRecord(p->ev_out_ready[o], p->s_compute));
+            LOOP_TRY(cudaStreamWaitEvent(p->s_d2h, p->ev_out_ready[o], 0));
+            LOOP_TRY(cudaEventRecord(p->ev_d2h_start[o], p->s_d2h));
+            LOOP_TRY(cudaMemcpyAsync(p->h_out[o], deliver, n_pix * sizeof(float), cudaMemcpyDeviceToHost, p->s_d2h));
+            LOOP_TRY(cudaEventRecord(p->ev_d2h_done[o], p->s_d2h));
             out_idx[o] = n;
             ++n_out;
             st.d2h_bytes += (double)(n_pix * sizeof(float));
@@ -935,6 +973,7 @@ int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *f
             if (src < 0) { rc = fail(p, TOI_ERR_CALLBACK, "sink callback failed"); break; }
         }
     }
+#undef LOOP_TRY
     cudaStreamSynchronize(p->s_copy);
     cudaStreamSynchronize(p->s_compute);
     if (p->s_d2h) cudaStreamSynchronize(p->s_d2h);
@@ -1027,8 +1066,7 @@ int toi_debug_cell_indices(toi_plan *p, int32_t *d_iu, int32_t *d_iv)
 int toi_debug_keep_grid(toi_plan *p, int32_t on)
 {
     if (!p) return fail(nullptr, TOI_ERR_INVALID_ARG, "plan is NULL");
-    CU_TRY(p, cudaSetDevice(p->cfg.device));
-    if (on && !p->d_grid_keep) CU_TRY(p, cudaMalloc(&p->d_grid_keep, (size_t)p->geo.G * p->geo.G * sizeof(float2)));
+    if (on && !p->d_grid_keep) return fail(p, TOI_ERR_UNSUPPORTED, "debug capture needs a plan created with debug_keep_grid = 1");
     p->keep_grid = on != 0;
     return TOI_OK;
 }
@@ -1046,10 +1084,11 @@ int toi_debug_copy_grid(toi_plan *p, void *d_grid_c64)
 int toi_debug_copy_density(toi_plan *p, float *d_density)
 {
     if (!p || !d_density) return fail(p, TOI_ERR_INVALID_ARG, "NULL argument");
-    if (!p->d_dens[0]) return fail(p, TOI_ERR_INVALID_ARG, "plan was not created with uniform weighting");
+    if (!p->d_dens) return fail(p, TOI_ERR_INVALID_ARG, "plan was not created with uniform weighting");
+    if (!p->keep_grid || !p->d_dens_keep) return fail(p, TOI_ERR_INVALID_ARG, "call toi_debug_keep_grid(plan, 1) before imaging");
     CU_TRY(p, cudaSetDevice(p->cfg.device));
     CU_TRY(p, cudaDeviceSynchronize());
-    CU_TRY(p, cudaMemcpy(d_density, p->d_dens[p->last_k], (size_t)p->geo.G * p->geo.G * sizeof(float), cudaMemcpyDeviceToDevice));
+    CU_TRY(p, cudaMemcpy(d_density, p->d_dens_keep, (size_t)p->geo.G * p->geo.G * sizeof(float), cudaMemcpyDeviceToDevice));
     return TOI_OK;
 }
 

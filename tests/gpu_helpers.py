@@ -17,7 +17,7 @@ class GpuImager:
 
     def __init__(self, snap, N, cell_size_deg, weighting="natural", gridder=toi.TOI_GRIDDER_SLIDING,
                  location=toi.TOI_MEM_DEVICE, pol_a=None, pol_b=None, grid_size=0, apply_jacobian=0,
-                 ring_depth=0):
+                 ring_depth=0, keep_grid=False, enable_3d=False):
         vis = snap["vis"]
         self.n_b, self.n_c, self.n_p = vis.shape
         self.N = N
@@ -27,7 +27,10 @@ class GpuImager:
         self.plan = toi.toi_plan_create(self.n_b, self.n_c, self.n_p, snap["chan_freq_hz"], N, cell_size_deg,
                                         weighting=wt, pol_a=pol_a, pol_b=pol_b, grid_size=grid_size,
                                         apply_jacobian=apply_jacobian, input_location=location,
-                                        image_ring_depth=ring_depth, gridder=gridder)
+                                        image_ring_depth=ring_depth, gridder=gridder, enable_3d=enable_3d,
+                                        debug_keep_grid=keep_grid)
+        if keep_grid:
+            toi.toi_debug_keep_grid(self.plan, True)
         self.set_inputs(snap)
 
     def set_inputs(self, snap):

@@ -68,7 +68,7 @@ def oracle_inputs(snap, V):
 def run_gpu(snap, N, cell, n_slab, K, weighting=toi.TOI_WEIGHT_NATURAL):
     n_b, n_c, n_p = snap["vis"].shape
     plan = toi.toi_plan_create(n_b, n_c, n_p, snap["chan_freq_hz"], N, cell, weighting=weighting,
-                               input_location=toi.TOI_MEM_DEVICE)
+                               input_location=toi.TOI_MEM_DEVICE, enable_3d=True)
     try:
         t = {k: (None if snap[k] is None else torch.from_numpy(np.ascontiguousarray(snap[k])).cuda())
              for k in ("uvw_m", "vis", "weights", "flags")}
@@ -144,7 +144,7 @@ def test_3d_mode_uniform_weighting_and_back_to_back_calls():
     N, cell = 64, 200.0 / 3600.0
     n_b, n_c, n_p = planar["vis"].shape
     plan = toi.toi_plan_create(n_b, n_c, n_p, planar["chan_freq_hz"], N, cell, weighting=toi.TOI_WEIGHT_UNIFORM,
-                               input_location=toi.TOI_MEM_DEVICE)
+                               input_location=toi.TOI_MEM_DEVICE, enable_3d=True)
     try:
         t = {k: (None if planar[k] is None else torch.from_numpy(np.ascontiguousarray(planar[k])).cuda())
              for k in ("uvw_m", "vis", "weights", "flags")}
@@ -174,7 +174,8 @@ def test_3d_mode_with_host_inputs_equals_device_inputs_and_refuses_bad_arguments
     N, cell = 64, 200.0 / 3600.0
     img_dev, i3_dev, info_dev, _ = run_gpu(snap, N, cell, 2, 8)
     n_b, n_c, n_p = snap["vis"].shape
-    plan = toi.toi_plan_create(n_b, n_c, n_p, snap["chan_freq_hz"], N, cell, input_location=toi.TOI_MEM_HOST)
+    plan = toi.toi_plan_create(n_b, n_c, n_p, snap["chan_freq_hz"], N, cell, input_location=toi.TOI_MEM_HOST,
+                               enable_3d=True)
     try:
         t = {k: (None if snap[k] is None else torch.from_numpy(np.ascontiguousarray(snap[k])).pin_memory())
              for k in ("uvw_m", "vis", "weights", "flags")}

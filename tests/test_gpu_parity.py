@@ -55,9 +55,8 @@ def _check_all(snap, wl_N, cell, weighting, gridder, pol_a=None, pol_b=None, loc
     rc, img_o, info_o, ex = _oracle(snap, wl_N, cell, weighting, pol_a=pol_a, pol_b=pol_b, want_grid=check_grid,
                                     want_density=(weighting == "uniform"), want_indices=True)
     assert rc == 0
-    with GpuImager(snap, wl_N, cell, weighting, gridder, location, pol_a, pol_b) as gi:
-        if check_grid:
-            toi.toi_debug_keep_grid(gi.plan, True)
+    with GpuImager(snap, wl_N, cell, weighting, gridder, location, pol_a, pol_b,
+                   keep_grid=check_grid or weighting == "uniform") as gi:
         # (i) own fit: V within 1e-12 of the oracle's explicit-B fit
         img_g, info_g, _ = gi.image()
         V_g = np.array(info_g["V"])
@@ -93,7 +92,7 @@ def _check_all(snap, wl_N, cell, weighting, gridder, pol_a=None, pol_b=None, loc
 # ------------------------------------------------------------------------------------------------
 # config 1 (BASELINE.json configs[0]): the tiny snapshot, natural weighting, both gridders
 # ------------------------------------------------------------------------------------------------
-ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_PAIR7, toi.TOI_GRIDDER_SLIDING7, toi.TOI_GRIDDER_ATOMIC]
+ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_ATOMIC]
 
 
 @pytest.mark.parametrize("gridder", ALL_GRIDDERS)
@@ -141,14 +140,14 @@ def test_reduced_config2(weighting, gridder):
 
 
 def test_reduced_config2_long_rows():
-    """More channels than one task covers (4 strips x 256): several tasks per baseline row."""
+    """More channels than one task covers (8 strips x 128): several tasks per baseline row."""
     wl = _reduced2(n_ant=12, n_chan=2500, image_size=1024)
     snap = snapshot_np(wl)
     _check_all(snap, wl.image_size, wl.cell_size_deg, "natural", toi.TOI_GRIDDER_SLIDING, pol_a=0, pol_b=3,
                check_grid=False)
 
 
-@pytest.mark.parametrize("gridder", [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_PAIR7, toi.TOI_GRIDDER_SLIDING7])
+@pytest.mark.parametrize("gridder", ALL_GRIDDERS)
 @pytest.mark.parametrize("weighting", ["natural", "uniform"])
 def test_coarse_channels_make_the_window_jump(gridder, weighting):
     """16 channels across the whole band: consecutive samples of a long baseline are tens of cells
@@ -257,9 +256,9 @@ def test_edge_image_size_not_a_multiple_of_8(image_size):
     _check_all(snap, wl.image_size, wl.cell_size_deg, "natural", toi.TOI_GRIDDER_SLIDING)
 
 
-def test_back_to_back_snapshots_alternate_grid_buffers():
-    """The grid / density buffers are a ring of 2 zero-filled on a side stream: five snapshots in a
-    row (uniform weighting) must all equal the first."""
+def test_back_to_back_snapshots_find_a_zero_grid():
+    """The grid / density map are cleared sparsely (only the tiles the snapshot touched) after the
+    first FFT pass: five snapshots in a row (uniform weighting) must all equal the first."""
     wl = _reduced2(n_ant=12, n_chan=130, image_size=256)
     snap = snapshot_np(wl)
     rc, img_o, _, _ = _oracle(snap, wl.image_size, wl.cell_size_deg, "uniform", pol_a=0, pol_b=3)
@@ -295,8 +294,7 @@ def test_edge_grid_half_size_odd_or_tight(G, gridder):
     assert rc == 0 and info_o["n_gridded"] > 0
     if G == 136:
         assert info_o["n_off_grid"] > 0
-    with GpuImager(snap, wl.image_size, wl.cell_size_deg, "natural", gridder, grid_size=G) as gi:
-        toi.toi_debug_keep_grid(gi.plan, True)
+    with GpuImager(snap, wl.image_size, wl.cell_size_deg, "natural", gridder, grid_size=G, keep_grid=True) as gi:
         img, info, _ = gi.image()
         grid = gi.grid_centred()
     assert info["n_gridded"] == info_o["n_gridded"] and info["n_off_grid"] == info_o["n_off_grid"]

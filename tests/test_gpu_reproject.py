@@ -276,7 +276,15 @@ def test_stream_output_refuses_bad_settings_and_propagates_host_sink_errors():
             toi.toi_stream_set_output(plan, product=9)
     finally:
         toi.toi_plan_destroy(plan)
-    wl, plan, fill, _ = _stream_case(4, ring=2)
+    wl, plan, fill, _ = _stream_case(3, ring=2)
+    try:
+        with pytest.raises(toi.ToiError) as ei:      # the D2H ring needs an image ring of depth >= 3
+            toi.toi_stream_set_output(plan, host_sink=lambda idx, image: 0, image_size=wl.image_size)
+        assert ei.value.code == toi.TOI_ERR_INVALID_ARG
+        toi.toi_stream_set_output(plan, difference=True)     # depth 2 is enough for the difference alone
+    finally:
+        toi.toi_plan_destroy(plan)
+    wl, plan, fill, _ = _stream_case(4, ring=3)
     try:
         toi.toi_stream_set_output(plan, host_sink=lambda idx, image: -1, image_size=wl.image_size)
         with pytest.raises(toi.ToiError) as ei:
