@@ -8,8 +8,11 @@ gridding, inverse FFT, correction + crop) on BASELINE.json configs[1]: one MeerK
 Prints ONE JSON line (rank 0).  `value` = visibilities (baseline-channel samples) gridded per second
 over all ranks with inputs resident in HBM; `e2e` = the same through the C ABI with pinned HOST
 buffers (H2D of every input and D2H of the image inside the timed region); `roofline` = the
-gridding kernel against the measured HBM copy rate; `cpu_baseline` = the fp64 oracle on the host
-cores.  --impl reference times the oracle itself (the only "reference" this paper-only task has).
+gridding kernel (+ the sparse clear of its grid) against the measured HBM copy rate;
+`roofline_natural` / `stages_ms_natural` = the same workload under the paper's own natural weighting;
+`workloads` = BASELINE.json configs[3] and configs[4] (natural); `stream` = configs[2], 1500 snapshots
+through toi_image_stream from a pinned pool of distinct snapshots; `cpu_baseline` = the fp64 oracle on
+the host cores.  --impl reference times the oracle itself (the only "reference" this paper-only task has).
 """
 from __future__ import annotations
 
@@ -30,6 +33,7 @@ import torch  # noqa: E402
 METRIC = "visibilities gridded per second, whole snapshot hot path (ms/snapshot in ms_per_step)"
 UNIT = "vis/s"
 PAPER_MS_PER_SNAPSHOT_H100 = 120.0   # PAPER.md:456, end to end incl. FITS writing: context only
+STAGE_KEYS = ["ms_planefit", "ms_weight", "ms_grid", "ms_fft", "ms_crop", "ms_total", "ms_clear"]
 
 
 def parse_args():
@@ -41,11 +45,15 @@ def parse_args():
     ap.add_argument("--workload", type=int, default=2, choices=[1, 2, 4, 5],
                     help="BASELINE.json config id (2 = configs[1], the metric's workload)")
     ap.add_argument("--weighting", default=None, choices=[None, "natural", "uniform"])
-    ap.add_argument("--gridder", default="sliding", choices=["sliding", "pair7", "sliding7", "atomic"])
-    ap.add_argument("--stream-snapshots", type=int, default=60,
-                    help="length of the streamed (config-3-shaped) run reported under `stream`; 0 = skip")
+    ap.add_argument("--gridder", default="sliding", choices=["sliding", "atomic", "ws"])
+    ap.add_argument("--stream-snapshots", type=int, default=1500,
+                    help="length of the streamed (configs[2]) run reported under `stream`; 0 = skip")
+    ap.add_argument("--stream-pool", type=int, default=16,
+                    help="distinct pinned snapshots the streamed run cycles through")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-snapshots", type=int, default=3)
+    ap.add_argument("--no-extra-workloads", action="store_true",
+                    help="skip the natural-weighting arm and configs[3] / configs[4]")
+    ap.add_argument("--cpu-snapshots", type=int, default=2)
     return ap.parse_args()
 
 
@@ -138,6 +146,7 @@ def algorithmic_bytes(wl, weighting):
 
 
 def config_dict(wl, weighting, args, world):
+    in_mb = wl.n_baselines * wl.n_chan * wl.n_pol * 13 / 1e6
     return {"workload": "BASELINE.json configs[%d] %s: %d baselines x %d channels x %d pols, %dx%d image, "
                         "G=%d, W=7, %s weighting, seeded synthetic (synth.py)" %
                         (wl.config_id - 1, wl.name, wl.n_baselines, wl.n_chan, wl.n_pol, wl.image_size,
@@ -145,29 +154,39 @@ def config_dict(wl, weighting, args, world):
             "samples_per_snapshot": wl.n_baselines * wl.n_chan,
             "input_bytes_per_snapshot": wl.n_baselines * wl.n_chan * wl.n_pol * 13 + wl.n_baselines * 24,
             "gridder": args.gridder,
-            "l2": "inputs (%.0f MB) larger than the 126 MB L2; no flush needed" %
-                  (wl.n_baselines * wl.n_chan * wl.n_pol * 13 / 1e6),
+            "l2": "inputs (%.0f MB) + grid and FFT workspace (2 x %.0f MB) streamed every step: far larger than "
+                  "the 126 MB L2; no flush needed" % (in_mb, (2 * wl.image_size) ** 2 * 8 / 1e6),
             "parallelism": "snapshots sharded over %d GPU(s), no collective" % world}
 
 
-def oracle_snapshot_seconds(snap_np, wl, weighting, repeats):
-    """The oracle as it stands (Tier G, fp64, OpenMP) on one snapshot, `repeats` times -> seconds each."""
+def oracle_snapshot_seconds(snap_np, wl, weighting, repeats, threads=None):
+    """The oracle as it stands (Tier G, fp64, OpenMP) on one snapshot, `repeats` times -> seconds each,
+    plus its own per-stage wall clock of the last call."""
     import oracle
     wt = oracle.UNIFORM if weighting == "uniform" else oracle.NATURAL
-    times = []
-    for _ in range(repeats):
-        t0 = time.perf_counter()
-        rc, _, info, _ = oracle.image_gridded(snap_np["uvw_m"], snap_np["vis"], snap_np["weights"], snap_np["flags"],
-                                              snap_np["chan_freq_hz"], wl.image_size, wl.cell_size_deg,
-                                              weighting=wt, pol_a=0, pol_b=wl.n_pol - 1)
-        times.append(time.perf_counter() - t0)
-        assert rc == 0
-    return times, int(info["n_gridded"]), oracle.num_threads()
+    all_cores = oracle.num_threads()
+    if threads:
+        oracle.set_num_threads(threads)
+    times, info = [], None
+    try:
+        for _ in range(repeats):
+            t0 = time.perf_counter()
+            rc, _, info, _ = oracle.image_gridded(snap_np["uvw_m"], snap_np["vis"], snap_np["weights"], snap_np["flags"],
+                                                  snap_np["chan_freq_hz"], wl.image_size, wl.cell_size_deg,
+                                                  weighting=wt, pol_a=0, pol_b=wl.n_pol - 1)
+            times.append(time.perf_counter() - t0)
+            assert rc == 0
+        stages = {k: 1e3 * v for k, v in oracle.last_stage_seconds().items()}
+        cores = oracle.num_threads()
+    finally:
+        if threads:
+            oracle.set_num_threads(all_cores)
+    return times, int(info["n_gridded"]), cores, stages
 
 
-def make_inputs(wl, device):
+def make_inputs(wl, device, snapshot=0):
     from paper_2512_06254_b200 import synth
-    return synth.make_snapshot(wl, 0, device=device)
+    return synth.make_snapshot(wl, snapshot, device=device)
 
 
 def run_reference(args):
@@ -183,7 +202,7 @@ def run_reference(args):
     steps = max(1, min(args.steps, 20))
     warm = max(0, min(args.warmup, 1))
     oracle_snapshot_seconds(snap_np, wl, weighting, max(1, warm))
-    times, n_gridded, cores = oracle_snapshot_seconds(snap_np, wl, weighting, steps)
+    times, n_gridded, cores, stages = oracle_snapshot_seconds(snap_np, wl, weighting, steps)
     ms = 1e3 * sum(times) / len(times)
     S = wl.n_baselines * wl.n_chan
     value = S / (ms * 1e-3)
@@ -191,11 +210,79 @@ def run_reference(args):
             "steps": steps, "warmup": max(1, warm), "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": config_dict(wl, weighting, args, 1),
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "stages_ms": stages,
                              "sample": "%d full snapshot(s) of the workload, one per step" % steps},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def time_stages(toi, plan, snap, stream, reps):
+    """Per-stage durations (CUDA events inside the library, on `stream`; every call synchronises)."""
+    acc = {k: [] for k in STAGE_KEYS}
+    info = None
+    for _ in range(reps):
+        _, info, _ = toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"],
+                                            stream=stream, want_info=True)
+        for k in STAGE_KEYS:
+            acc[k].append(getattr(info, k))
+    return ({k: sum(v) / len(v) for k, v in acc.items()}, {k: min(v) for k, v in acc.items()}, int(info.n_gridded))
+
+
+def time_3d(toi, plan, snap, stream, reps=3):
+    """Near-coplanar 3-D mode (NEXT-2): N_slab x K Chebyshev-moment passes, parameters chosen from the
+    snapshot (Eqs. 25-27); the call synchronises once, so its own CUDA-event time is reported."""
+    toi.toi_image_snapshot_3d(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
+    t3d, i3 = [], None
+    for _ in range(reps):
+        _, i3, _ = toi.toi_image_snapshot_3d(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
+        t3d.append(i3["ms_total"])
+    return {"ms": sum(t3d) / len(t3d), "ms_min": min(t3d), "n_slab": i3["n_slab"], "K": i3["K"], "passes": i3["n_passes"],
+            "phi_max": i3["phi_max"], "expansion_error": i3["expansion_error"]}
+
+
+def roofline_of(wl, weighting, stages, stages_min, peak, peak_src, kernel):
+    """Gridding against the HBM roofline: algorithmic bytes (every input byte once + the grid once) over
+    the gridding kernel + the sparse clear of its grid, both timed in situ with CUDA events."""
+    ab = algorithmic_bytes(wl, weighting)
+    grid_ms = stages["ms_grid"] + stages["ms_clear"]
+    achieved = ab["gridding"] / (grid_ms * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": kernel + " + k_clear_tiles (sparse clear of the grid, and of the density map)",
+            "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "frac_of_8tbs_nominal": achieved / 8000.0, "peak_source": peak_src,
+            "algorithmic_bytes": ab["gridding"], "ms": grid_ms, "ms_kernel": stages["ms_grid"],
+            "ms_clear": stages["ms_clear"], "ms_kernel_min": stages_min["ms_grid"],
+            "vis_per_s": ab["samples"] / (grid_ms * 1e-3)}
+
+
+def run_side_workload(toi, wl, weighting, local, gridder, stream, steps, with_3d):
+    """One more (workload, weighting) pair, device-resident: whole-step time + stages.  Rank 0 only."""
+    snap = make_inputs(wl, "cuda")
+    freq = snap["chan_freq_hz"].cpu()
+    wt = toi.TOI_WEIGHT_UNIFORM if weighting == "uniform" else toi.TOI_WEIGHT_NATURAL
+    plan = toi.toi_plan_create(wl.n_baselines, wl.n_chan, wl.n_pol, freq, wl.image_size, wl.cell_size_deg, weighting=wt,
+                               pol_a=0, pol_b=wl.n_pol - 1, input_location=toi.TOI_MEM_DEVICE, device=local,
+                               gridder=gridder, enable_3d=with_3d)
+    try:
+        def step():
+            toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
+        for _ in range(3):
+            step()
+        toi.toi_plan_sync(plan)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms_step = e0.elapsed_time(e1) / steps
+        stages, stages_min, n_gridded = time_stages(toi, plan, snap, stream, max(5, min(steps, 20)))
+        m3 = time_3d(toi, plan, snap, stream) if with_3d else None
+    finally:
+        toi.toi_plan_destroy(plan)
+        del snap
+        torch.cuda.empty_cache()
+    return ms_step, stages, stages_min, n_gridded, m3
 
 
 def run_ours(args):
@@ -210,8 +297,7 @@ def run_ours(args):
     toi.load()
     wl, weighting = workload(args)
     wt = toi.TOI_WEIGHT_UNIFORM if weighting == "uniform" else toi.TOI_WEIGHT_NATURAL
-    gridder = {"sliding": toi.TOI_GRIDDER_SLIDING, "pair7": toi.TOI_GRIDDER_PAIR7, "sliding7": toi.TOI_GRIDDER_SLIDING7,
-               "atomic": toi.TOI_GRIDDER_ATOMIC}[args.gridder]
+    gridder = {"sliding": toi.TOI_GRIDDER_SLIDING, "atomic": toi.TOI_GRIDDER_ATOMIC, "ws": toi.TOI_GRIDDER_WS}[args.gridder]
     S = wl.n_baselines * wl.n_chan
     N = wl.image_size
     snap = make_inputs(wl, "cuda")            # seeded generator, on the device; every rank the same shape
@@ -219,9 +305,10 @@ def run_ours(args):
     stream = torch.cuda.Stream()
 
     # ---------------- device-resident arm: `value` ----------------
+    with_3d = args.gridder != "atomic"
     plan = toi.toi_plan_create(wl.n_baselines, wl.n_chan, wl.n_pol, freq, N, wl.cell_size_deg, weighting=wt,
                                pol_a=0, pol_b=wl.n_pol - 1, input_location=toi.TOI_MEM_DEVICE, device=local,
-                               gridder=gridder)
+                               gridder=gridder, enable_3d=with_3d)
 
     def step():
         toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
@@ -250,18 +337,7 @@ def run_ours(args):
     ms_step = ms_total / args.steps
     value = units / (ms_total * 1e-3)
 
-    # ---------------- per-stage durations (CUDA events inside the library, on `stream`) ----------------
-    stage_keys = ["ms_planefit", "ms_weight", "ms_grid", "ms_fft", "ms_crop", "ms_total", "ms_zero"]
-    acc = {k: [] for k in stage_keys}
-    info = None
-    for _ in range(max(5, min(args.steps, 20))):
-        _, info, _ = toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"],
-                                            stream=stream, want_info=True)
-        for k in stage_keys:
-            acc[k].append(getattr(info, k))
-    stages = {k: sum(v) / len(v) for k, v in acc.items()}
-    stages_min = {k: min(v) for k, v in acc.items()}
-    n_gridded = int(info.n_gridded)
+    stages, stages_min, n_gridded = time_stages(toi, plan, snap, stream, max(5, min(args.steps, 20)))
     # ---------------- NEXT rows, timed on their own (not part of `value`): re-projection of the
     # image just made with the snapshot's own V, and the difference of two ring images ----------------
     ptr_a, _, _ = toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
@@ -284,32 +360,12 @@ def run_ours(args):
         extra[name] = tot / reps
         extra[name + "_min"] = best
     del out_img
-    # near-coplanar 3-D mode (NEXT-2): N_slab x K Chebyshev-moment passes, parameters chosen from the
-    # snapshot (Eqs. 25-27); the call synchronises once, so its own CUDA-event time is reported
-    toi.toi_image_snapshot_3d(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
-    t3d = []
-    for _ in range(3):
-        _, i3, _ = toi.toi_image_snapshot_3d(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream)
-        t3d.append(i3["ms_total"])
-    extra["mode_3d"] = {"ms": sum(t3d) / len(t3d), "n_slab": i3["n_slab"], "K": i3["K"], "passes": i3["n_passes"],
-                        "phi_max": i3["phi_max"], "expansion_error": i3["expansion_error"]}
+    if with_3d:
+        extra["mode_3d"] = time_3d(toi, plan, snap, stream)
     toi.toi_plan_destroy(plan)
-    # the grid's zero fill alone (same size, same API call the library uses), best of 5
-    zbuf = torch.empty(4 * N * N * 2, dtype=torch.float32, device="cuda")   # G x G complex64
-    zero_alone_ms = 1e9
-    for _ in range(6):
-        z0, z1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        z0.record(stream)
-        with torch.cuda.stream(stream):
-            zbuf.zero_()
-        z1.record(stream)
-        torch.cuda.synchronize()
-        zero_alone_ms = min(zero_alone_ms, z0.elapsed_time(z1))
-    del zbuf
     return dict(rank=rank, local=local, world=world, wl=wl, weighting=weighting, wt=wt, gridder=gridder, S=S, N=N,
                 snap=snap, freq=freq, stream=stream, ms_step=ms_step, value=value, clocks=clocks, stages=stages,
-                stages_min=stages_min, n_gridded=n_gridded, launches_per_step=launches_per_step,
-                zero_alone_ms=zero_alone_ms, extra=extra)
+                stages_min=stages_min, n_gridded=n_gridded, launches_per_step=launches_per_step, extra=extra)
 
 
 def pinned_h2d_peak_gbs(n_bytes=1 << 30, repeats=5):
@@ -333,6 +389,7 @@ def run_e2e(r, args):
     reads the image back D2H inside the timed region."""
     from paper_2512_06254_b200 import binding as toi
     from paper_2512_06254_b200 import shard
+    from paper_2512_06254_b200 import synth
     wl, snap, stream, N = r["wl"], r["snap"], r["stream"], r["N"]
     host = {k: (snap[k].cpu().pin_memory() if snap[k] is not None else None)
             for k in ("uvw_m", "vis", "weights", "flags")}
@@ -368,31 +425,56 @@ def run_e2e(r, args):
            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
            "h2d_gbs_per_gpu": h2d * steps / (ms * 1e-3) / 1e9}
 
-    # streamed run (config-3-shaped): pinned replay pool -> copy stream -> compute stream, events only
+    # streamed run, BASELINE.json configs[2]: `--stream-snapshots` (1500) consecutive toi_image_stream
+    # snapshots fed from a pinned pool of `--stream-pool` DISTINCT snapshots of the run (evenly spaced
+    # indices: hour angle advancing, pulsar on and off), generated on the GPU by the seeded generator
+    # and copied into pinned host memory before the timed region; pinned ring -> copy stream ->
+    # compute stream, events only.  1500 x 429.5 MB cannot be held, so the stream cycles through the pool.
     stream_res = None
-    if args.stream_snapshots > 0 and r["rank"] == 0:
+    if args.stream_snapshots > 0 and r["rank"] == 0 and wl.config_id == 2:
+        w3 = synth.CONFIG3
+        n_pool = max(1, min(args.stream_pool, args.stream_snapshots))
+        idxs = sorted({int(round(k * (w3.n_snapshots - 1) / max(1, n_pool - 1))) for k in range(n_pool)})
+        pool = []
+        t_gen = time.perf_counter()
+        for i in idxs:
+            d = make_inputs(w3, "cuda", snapshot=i)
+            pool.append({k: (d[k].cpu().pin_memory() if d[k] is not None else None)
+                         for k in ("uvw_m", "vis", "weights", "flags")})
+            del d
+        torch.cuda.empty_cache()
+        t_gen = time.perf_counter() - t_gen
+
         def fill(idx, slot):
-            slot.uvw_m = host["uvw_m"].data_ptr()
-            slot.vis = host["vis"].data_ptr()
-            slot.weights = host["weights"].data_ptr() if host["weights"] is not None else None
-            slot.flags = host["flags"].data_ptr() if host["flags"] is not None else None
+            h = pool[idx % len(pool)]
+            slot.uvw_m = h["uvw_m"].data_ptr()
+            slot.vis = h["vis"].data_ptr()
+            slot.weights = h["weights"].data_ptr() if h["weights"] is not None else None
+            slot.flags = h["flags"].data_ptr() if h["flags"] is not None else None
             return 0
         toi.toi_image_stream(plan, 4, fill)                     # warm-up
         st = toi.toi_image_stream(plan, args.stream_snapshots, fill)
-        stream_res = {"snapshots": int(st["n_done"]), "ms_per_snapshot": st["gpu_ms"] / max(1, st["n_done"]),
-                      "wall_ms_per_snapshot": 1e3 * st["wall_s"] / max(1, st["n_done"]),
+        n_done = max(1, int(st["n_done"]))
+        stream_res = {"workload": "BASELINE.json configs[2] meerkat_stream: config 2's layout, %d snapshots 2 s apart, "
+                                  "on/off 5 mJy pulsar, uniform weighting" % w3.n_snapshots,
+                      "snapshots": int(st["n_done"]), "ms_per_snapshot": st["gpu_ms"] / n_done,
+                      "seconds_total_gpu_events": st["gpu_ms"] * 1e-3, "seconds_total_wall": st["wall_s"],
+                      "wall_ms_per_snapshot": 1e3 * st["wall_s"] / n_done,
                       "h2d_gbs": st["h2d_bytes"] / (st["gpu_ms"] * 1e-3) / 1e9,
-                      "h2d_ms_mean": st["h2d_ms_sum"] / max(1, st["n_done"]),
-                      "compute_ms_mean": st["compute_ms_sum"] / max(1, st["n_done"]),
-                      "source": "replay pool of 1 pinned snapshot (DESIGN.md section 4); images stay on the GPU"}
+                      "h2d_ms_mean": st["h2d_ms_sum"] / n_done,
+                      "compute_ms_mean": st["compute_ms_sum"] / n_done,
+                      "pool": {"distinct_snapshots": len(pool), "snapshot_indices": idxs,
+                               "pinned_bytes": len(pool) * h2d, "generate_s": t_gen},
+                      "source": "pinned pool of distinct seeded snapshots, cycled (DESIGN.md section 4); images stay on the GPU"}
         # the same stream with the output side on: re-projection of every image (interpolate stage)
         # and its D2H through the pinned ring to a host sink (copy_cpu stage)
         seen = []
+        n_out = max(4, min(args.stream_snapshots, 300))
         toi.toi_stream_set_output(plan, product=toi.TOI_OUT_REPROJECT_EXACT,
                                   host_sink=lambda idx, image: seen.append(idx), image_size=N)
         toi.toi_image_stream(plan, 4, fill)
         del seen[:]
-        st = toi.toi_image_stream(plan, args.stream_snapshots, fill)
+        st = toi.toi_image_stream(plan, n_out, fill)
         stream_res["with_output"] = {
             "snapshots": int(st["n_done"]), "images_on_host": len(seen),
             "ms_per_snapshot": st["gpu_ms"] / max(1, st["n_done"]),
@@ -402,25 +484,21 @@ def run_e2e(r, args):
             "d2h_ms_mean": st["d2h_ms_sum"] / max(1, st["n_done"]),
             "what": "re-projected (exact) image of every snapshot delivered to a host callback"}
         toi.toi_stream_set_output(plan)
+        del pool
     toi.toi_plan_destroy(plan)
     return e2e, stream_res
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
-# `ncu --set full` captures summarised under profiles/ (a recorded measurement of the same command,
-# not something this run can observe).  The 134 MB grid zero fill is a separate cudaMemsetAsync and
-# most of the reductions stay in the 126 MB L2 until the FFT reads them, hence the small write figure.
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel: read off the
+# `ncu --set full` capture named in `source` (a recorded measurement of the same command line, taken
+# on `date`; this run cannot observe DRAM counters itself).  The sparse clear is a separate launch,
+# and most of the reductions stay in the 126 MB L2 until the FFT reads them, hence the small write figure.
 NCU_TRAFFIC = {
-    ("2", "uniform", "sliding"): {"bytes": 471329280 + 5403136, "source": "profiles/r1_k_grid_pair8_full.txt"},
-    ("2", "natural", "sliding"): {"bytes": 459540992 + 5927424, "source": "profiles/r1_k_grid_pair8_natural_full.txt"},
-    ("2", "uniform", "pair7"): {"bytes": 473425920 + 5772032, "source": "profiles/r1_k_grid_pair_full.txt"},
-    ("2", "uniform", "sliding7"): {"bytes": 461792768 + 6813696, "source": "profiles/r1_k_grid_sliding_full.txt"},
+    ("2", "uniform", "sliding"): {"bytes": 471329280 + 5403136, "source": "profiles/r1_k_grid_pair8_full.txt",
+                                  "date": "round 1 (before the round-2 kernel changes)"},
+    ("2", "natural", "sliding"): {"bytes": 459540992 + 5927424, "source": "profiles/r1_k_grid_pair8_natural_full.txt",
+                                  "date": "round 1 (before the round-2 kernel changes)"},
 }
-
-
-def ncu_traffic(args, weighting):
-    t = NCU_TRAFFIC.get((str(args.workload), weighting, args.gridder))
-    return None if t is None else t["bytes"]
 
 
 def main():
@@ -428,6 +506,8 @@ def main():
     if args.impl == "reference":
         run_reference(args)
         return
+    from paper_2512_06254_b200 import binding as toi
+    from paper_2512_06254_b200 import synth
     r = run_ours(args)
     e2e, stream_res = run_e2e(r, args)
     rank, world, wl, weighting = r["rank"], r["world"], r["wl"], r["weighting"]
@@ -441,21 +521,14 @@ def main():
         return
     ab = algorithmic_bytes(wl, weighting)
     peak, peak_src = measured_peaks()
-    # gridding kernel (CUDA events on its stream, while the side stream zero-fills the next
-    # snapshot's buffers under it) + the zero fill of one grid timed alone with CUDA events: the fill
-    # overlaps the kernels of the previous snapshot, so its in-situ duration (ms_zero) is not a cost
-    zero_alone_ms = r["zero_alone_ms"]
-    grid_ms = r["stages"]["ms_grid"] + zero_alone_ms
-    achieved = ab["gridding"] / (grid_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "%s (+ grid zero fill on the side stream)" % {"sliding": "k_grid_pair8", "pair7": "k_grid_pair", "sliding7": "k_grid_sliding", "atomic": "k_grid_atomic"}[args.gridder], "achieved": achieved,
-                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "frac_of_8tbs_nominal": achieved / 8000.0,
-                "peak_source": peak_src, "traffic": ncu_traffic(args, weighting),
-                "algorithmic_bytes": ab["gridding"], "ms": grid_ms, "ms_kernel": r["stages"]["ms_grid"],
-                "ms_zero_fill_alone": zero_alone_ms, "ms_zero_fill_in_situ": r["stages"]["ms_zero"], "ms_min": r["stages_min"]["ms_grid"],
-                "vis_per_s": r["S"] / (grid_ms * 1e-3)}
+    kernel = {"sliding": "k_grid_pair8", "atomic": "k_grid_atomic", "ws": "k_grid_ws"}[args.gridder]
+    roofline = roofline_of(wl, weighting, r["stages"], r["stages_min"], peak, peak_src, kernel)
+    tr = NCU_TRAFFIC.get((str(args.workload), weighting, args.gridder))
+    roofline["traffic"] = None if tr is None else tr["bytes"]
+    roofline["traffic_source"] = None if tr is None else "%s, %s" % (tr["source"], tr["date"])
     stages = {k: round(v, 5) for k, v in r["stages"].items()}
     if weighting == "uniform" and r["stages"]["ms_weight"] > 0:
-        stages["density_gbs"] = ab["density"] / ((r["stages"]["ms_weight"] + 0.5 * zero_alone_ms) * 1e-3) / 1e9
+        stages["density_gbs"] = ab["density"] / (r["stages"]["ms_weight"] * 1e-3) / 1e9
     stages["fft_gbs_min_traffic"] = ab["fft_min"] / (r["stages"]["ms_fft"] * 1e-3) / 1e9
     stages["crop_gbs"] = ab["crop"] / (r["stages"]["ms_crop"] * 1e-3) / 1e9
     # NEXT rows, timed alone: N^2 x (4 read + 4 written) resp. (8 read + 4 written)
@@ -464,20 +537,55 @@ def main():
     stages["reproject_gbs"] = n2 * 8 / (r["extra"]["ms_reproject_min"] * 1e-3) / 1e9
     stages["ms_difference"] = round(r["extra"]["ms_difference"], 5)
     stages["difference_gbs"] = n2 * 12 / (r["extra"]["ms_difference_min"] * 1e-3) / 1e9
-    stages["mode_3d"] = r["extra"]["mode_3d"]
+    stages["mode_3d"] = r["extra"].get("mode_3d")
     pcie = pinned_h2d_peak_gbs()
     e2e["pcie_peak_gbs_measured"] = pcie
     e2e["pcie_frac"] = e2e["h2d_gbs_per_gpu"] / pcie
     if stream_res is not None:
         stream_res["pcie_frac"] = stream_res["h2d_gbs"] / pcie
-        stream_res["extrapolated_s_for_1500_snapshots"] = 1.5 * stream_res["ms_per_snapshot"]
+
+    # ---------------- the paper's own weighting on the same workload, and the other configs ----------------
+    line_extra = {}
+    if not args.no_extra_workloads and args.workload == 2:
+        other = "natural" if weighting == "uniform" else "uniform"
+        ms_o, st_o, stmin_o, ng_o, _ = run_side_workload(toi, wl, other, r["local"], r["gridder"], r["stream"],
+                                                         args.steps, False)
+        line_extra["ms_per_step_" + other] = ms_o
+        line_extra["stages_ms_" + other] = {k: round(v, 5) for k, v in st_o.items()}
+        rf = roofline_of(wl, other, st_o, stmin_o, peak, peak_src, kernel)
+        tro = NCU_TRAFFIC.get((str(args.workload), other, args.gridder))
+        rf["traffic"] = None if tro is None else tro["bytes"]
+        rf["traffic_source"] = None if tro is None else "%s, %s" % (tro["source"], tro["date"])
+        line_extra["roofline_" + other] = rf
+        wls = []
+        for cid in (4, 5):
+            w = synth.CONFIGS[cid]
+            ms_w, st_w, stmin_w, ng_w, m3 = run_side_workload(toi, w, "natural", r["local"], r["gridder"], r["stream"],
+                                                              max(5, min(args.steps, 10)), cid == 5 and args.gridder != "atomic")
+            rw = roofline_of(w, "natural", st_w, stmin_w, peak, peak_src, kernel)
+            entry = {"workload": config_dict(w, "natural", args, 1)["workload"], "ms_per_step": ms_w,
+                     "value": w.n_baselines * w.n_chan / (ms_w * 1e-3), "unit": UNIT,
+                     "stages_ms": {k: round(v, 5) for k, v in st_w.items()}, "n_gridded": ng_w,
+                     "ms_grid": st_w["ms_grid"], "ms_clear": st_w["ms_clear"], "frac": rw["frac"],
+                     "frac_of_8tbs_nominal": rw["frac_of_8tbs_nominal"], "achieved_gbs": rw["achieved"],
+                     "algorithmic_bytes": rw["algorithmic_bytes"]}
+            if m3 is not None:
+                entry["mode_3d"] = m3
+            wls.append(entry)
+        line_extra["workloads"] = wls
+
     cpu = None
     if not args.no_cpu_baseline:
         snap_np = {k: (v.cpu().numpy() if v is not None else None) for k, v in r["snap"].items()}
-        times, _, cores = oracle_snapshot_seconds(snap_np, wl, weighting, max(1, args.cpu_snapshots))
+        times, _, cores, st_all = oracle_snapshot_seconds(snap_np, wl, weighting, max(1, args.cpu_snapshots))
         sec = sum(times) / len(times)
+        t1, _, _, st_one = oracle_snapshot_seconds(snap_np, wl, weighting, 1, threads=1)
         cpu = {"value": r["S"] / sec, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_snapshot": sec * 1e3,
-               "sample": "%d full snapshot(s) of the same workload (fp64 Tier G oracle, OpenMP)" % len(times)}
+               "stages_ms": {k: round(v, 2) for k, v in st_all.items()},
+               "one_thread": {"ms_per_snapshot": t1[0] * 1e3, "value": r["S"] / t1[0],
+                              "stages_ms": {k: round(v, 2) for k, v in st_one.items()}},
+               "sample": "%d full snapshot(s) of the same workload on all cores + 1 on one thread "
+                         "(fp64 Tier G oracle, OpenMP; its own per-stage wall clock)" % len(times)}
     line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": r["ms_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config_dict(wl, weighting, args, world),
@@ -486,6 +594,7 @@ def main():
             "n_gridded_per_snapshot": r["n_gridded"],
             "context": {"paper_ms_per_snapshot_h100_end_to_end": PAPER_MS_PER_SNAPSHOT_H100,
                         "note": "PAPER.md:456, 1770 bl x 1024 ch incl. FITS writing; not the target"}}
+    line.update(line_extra)
     print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist

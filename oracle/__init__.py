@@ -228,6 +228,13 @@ def image_dft(uvw_m, vis, weights, flags, chan_freq_hz, N, cell_size_deg, **kw):
     return rc, re.reshape(N, N), im.reshape(N, N), info
 
 
+def last_stage_seconds():
+    """Wall-clock seconds of the last image_gridded call per stage (instrumentation only)."""
+    out = (C.c_double * 5)()
+    lib().toi_oracle_last_stage_seconds(out)
+    return dict(zip(("fit", "weight", "grid", "fft", "correct"), [float(x) for x in out]))
+
+
 def num_threads():
     return int(lib().toi_oracle_num_threads())
 

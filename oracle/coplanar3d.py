@@ -119,6 +119,26 @@ def image_3d_direct(r, vis, V, omega, N, cell_size_deg, wsum=None):
     return img / norm
 
 
+def image_3d_direct_pixels(r, vis, V, omega, N, cell_size_deg, pix_i, pix_j, wsum=None, chunk=1 << 18):
+    """Eq. 18 at the listed pixels only (i = column, j = row), for inputs too large for the full image:
+    the same sum as image_3d_direct, pixel by pixel.  -> complex [n_pix] (NaN outside the sphere constraint)."""
+    beta = np.radians(cell_size_deg)
+    pix_i = np.asarray(pix_i, dtype=np.int64).ravel()
+    pix_j = np.asarray(pix_j, dtype=np.int64).ravel()
+    t1 = -beta * (pix_i - (N // 2)).astype(np.float64)
+    t2 = beta * (pix_j - (N // 2)).astype(np.float64)
+    t3 = t3_of(V, t1, t2)
+    r = np.asarray(r, dtype=np.float64)
+    vis = np.asarray(vis, dtype=np.complex128)
+    norm = omega * (vis.size if wsum is None else wsum)
+    out = np.zeros(pix_i.size, np.complex128)
+    for q0 in range(0, vis.size, chunk):
+        rq, vq = r[q0:q0 + chunk], vis[q0:q0 + chunk]
+        ph = rq[:, 0:1] * t1[None, :] + rq[:, 1:2] * t2[None, :] + rq[:, 2:3] * t3[None, :]     # [n, n_pix]
+        out += vq @ np.exp(2j * np.pi * ph)
+    return out / norm
+
+
 def image_3d_chebyshev(r, vis, V, omega, N, cell_size_deg, n_slab, K, wsum=None):
     """Eqs. 19-24 step by step: slabs, s_q, moments M_{p,k} (each a 2-D Fourier sum, Eq. 24), then
     I = 1/(omega N_vis) sum_p exp(i 2 pi r3_p t3) sum_k c_k(2 pi Delta_r3 t3) M_{p,k} (Eq. 23)."""

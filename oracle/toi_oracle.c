@@ -31,6 +31,7 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#include <time.h>
 #ifdef _OPENMP
 #include <omp.h>
 #endif
@@ -483,12 +484,29 @@ static void orc_density(const orc_config *cfg, int32_t G, int32_t W, const doubl
  *   iu_out, iv_out [n_b][n_c] int32 centre cells
  *   V_in       inject the transform instead of fitting it (index-parity protocol G5)
  * ---------------------------------------------------------------------------------------- */
+/* Wall-clock seconds the last toi_oracle_image_gridded call spent in each stage: plane fit + rotation,
+ * cell indices + weighting (density, counts, Wsum), gridding, FFT, correction + crop.  Read by
+ * bench.py's cpu_baseline; instrumentation only -- no arithmetic depends on it. */
+static double orc_stage_s[5];
+static double orc_now(void)
+{
+#ifdef _OPENMP
+    return omp_get_wtime();
+#else
+    return (double)clock() / CLOCKS_PER_SEC;
+#endif
+}
+void toi_oracle_last_stage_seconds(double out[5]) { memcpy(out, orc_stage_s, sizeof orc_stage_s); }
+
 int toi_oracle_image_gridded(const orc_config *cfg, const double *chan_freq_hz, const double *uvw_m,
                              const orc_c64 *vis, const float *weights, const uint8_t *flags,
                              const double *V_in, double *image, orc_info *info_out,
                              orc_c128 *grid_out, double *dens_out, int32_t *iu_out, int32_t *iv_out)
 {
     int32_t G, W;
+    double t_mark = orc_now(), t_now;
+    memset(orc_stage_s, 0, sizeof orc_stage_s);
+#define ORC_STAGE(k) (t_now = orc_now(), orc_stage_s[k] += t_now - t_mark, t_mark = t_now)
     if (!cfg || !chan_freq_hz || !uvw_m || !vis || !image) return ORC_ERR_ARG;
     int rc = orc_resolve(cfg, &G, &W);
     if (rc) return rc;
@@ -497,6 +515,7 @@ int toi_oracle_image_gridded(const orc_config *cfg, const double *chan_freq_hz, 
     double *s = NULL, *rho = NULL;
     rc = orc_front(cfg, chan_freq_hz, uvw_m, V_in, &s, &rho, &info);
     if (rc) { if (info_out) *info_out = info; return rc; }
+    ORC_STAGE(0);
     const double kappa = toi_oracle_kappa(G, cfg->cell_size_deg);
     const int64_t S = (int64_t)cfg->n_b * cfg->n_c;
 
@@ -528,6 +547,7 @@ int toi_oracle_image_gridded(const orc_config *cfg, const double *chan_freq_hz, 
         }
         info.wsum = (double)wsum;
     }
+    ORC_STAGE(1);
 
     /* Step 7. scatter: grid[iv+dv][iu+du] += f z phi(iu+du-gu) phi(iv+dv-gv), |du|,|dv| <= h.
      * Threads own bands of grid rows; every thread walks the samples in q order, so each
@@ -591,6 +611,7 @@ int toi_oracle_image_gridded(const orc_config *cfg, const double *chan_freq_hz, 
         }
         free(rowcount); free(edge);
     }
+    ORC_STAGE(2);
     if (grid_out) memcpy(grid_out, grid, (size_t)G * G * sizeof(orc_c128));
     if (dens_out) { if (D) memcpy(dens_out, D, (size_t)G * G * sizeof(double)); else memset(dens_out, 0, (size_t)G * G * sizeof(double)); }
     if (iu_out) memcpy(iu_out, iu, (size_t)S * sizeof(int32_t));
@@ -607,6 +628,7 @@ int toi_oracle_image_gridded(const orc_config *cfg, const double *chan_freq_hz, 
                 a[(int64_t)((kv + G) % G) * G + ((ku + G) % G)] = grid[(int64_t)(kv + G / 2) * G + (ku + G / 2)];
         rc = toi_oracle_fft2(a, G, +1);
         if (rc) { free(a); goto done; }
+        ORC_STAGE(3);
         /* Step 9. image = Re F / (psi(i-N/2) psi(j-N/2) omega Wsum)  (G7, G8, G11) */
         double *ipsi = (double *)malloc((size_t)N * sizeof(double));
         if (!ipsi) { free(a); rc = ORC_ERR_NOMEM; goto done; }
@@ -619,7 +641,9 @@ int toi_oracle_image_gridded(const orc_config *cfg, const double *chan_freq_hz, 
                 image[(int64_t)jj * N + ii] = info.wsum > 0.0 ? F.re / (ipsi[ii] * ipsi[jj] * norm) : 0.0;
             }
         free(ipsi); free(a);
+        ORC_STAGE(4);
     }
+#undef ORC_STAGE
 done:
     if (info_out) *info_out = info;
     free(iu); free(iv); free(on); free(grid); free(D); free(s); free(rho);

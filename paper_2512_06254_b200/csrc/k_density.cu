@@ -88,8 +88,12 @@ k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__rest
             atomicAdd(Dc + o, sum);
             atomicAdd(Dc - o, sum);                       // the mirror cell (-iu, -iv)
             // sparse clear (k_clear.cu): the tiles of the two cells just written
-            tiles[((iv + h) / kTile) * tpr + (iu + h) / kTile] = 1;
-            tiles[((h - iv) / kTile) * tpr + (h - iu) / kTile] = 1;
+            // (checked first: an L1 hit instead of a store that thousands of runs would send to the
+            // same few L2 sectors; a stale 0 only repeats the store)
+            uint8_t *const ta = tiles + ((iv + h) / kTile) * tpr + (iu + h) / kTile;
+            uint8_t *const tb = tiles + ((h - iv) / kTile) * tpr + (h - iu) / kTile;
+            if (*ta == 0) *ta = 1;
+            if (*tb == 0) *tb = 1;
         }
     }
 }

@@ -19,257 +19,15 @@
 // predicated on a predicate ptxas cannot see through (`pad == 0`), which keeps it from renaming the
 // accumulators and paying 10 MOVs per record on the fast path.
 
-#include "toi_internal.cuh"
+#include "grid_window.cuh"
+
 
 namespace toi {
 namespace {
 
-constexpr int kGroups = 8;        // 4-lane groups per warp
-constexpr int kBatch = 4;         // samples per group per pre-processing batch (8 * 4 = 32 lanes)
 constexpr int kWarps = 8;         // warps per CTA
-constexpr int kR = 8;             // rows (and column slots) of the register window
 constexpr int ctas_per_sm(bool) { return 2; }          // 16 warps/SM at <= 128 registers (4 x 4 warps measured 1 % slower)
-constexpr int kRecQuads = 5;      // record = 5 x 16 B: {zre, zim, wkey, pv0} {pv1..4} {pv5..7, 0} {pu0..3} {pu4..7}
-constexpr int kGroupQuads = kBatch * kRecQuads;          // 20; group g sits at quad 20 g + (g >> 1):
-constexpr int kWarpQuads = kGroups * kGroupQuads + 4;    // conflict-free STS.128 / LDS.128, spread tap words
-constexpr unsigned kNoKey = 0x80008000u;   // (bv, bu) = (-32768, -32768): never a window base (G <= 32768)
 
-constexpr int kHasW = 1, kHasF = 2, kHasD = 4;
-
-__device__ __forceinline__ unsigned cell_key(int iu, int iv) { return ((unsigned)iv << 16) | ((unsigned)iu & 0xffffu); }
-__device__ __forceinline__ int group_quad(int g) { return g * kGroupQuads + (g >> 1); }
-
-// ---- the consume phase: one group of 4 lanes, 4 records ------------------------------------------
-// Operands: %0..%7 rows of column set A, %8..%15 rows of set B, %16 tapA = window column my set A holds
-// (0..7; set B holds tapA ^ 4), %17 ckey = packed base cell of the open window (kNoKey: closed),
-// %18 / %19 = shared addresses of my A / B phi_u tap in record 0, %20 rgs = shared address of the
-// group's records, %21 gc = &grid cell (0,0), %22 row stride in bytes, %23 G, %24 L = lane in group.
-#define TOI8_HEAD(P, OFF)                                                                             \
-    "ld.shared.v4.b32 {zx" #P ", zy" #P ", key" #P ", va" #P "}, [%20+" #OFF "];\n\t"                \
-    "ld.shared.b32 pa" #P ", [%18+" #OFF "];\n\t"                                                     \
-    "ld.shared.b32 pb" #P ", [%19+" #OFF "];\n\t"
-#define TOI8_ROW(V, A, B)                                                                             \
-    "mov.b64 bb, {" V ", " V "};\n\tfma.rn.f32x2 " A ", ta, bb, " A ";\n\tfma.rn.f32x2 " B ", tb, bb, " B ";\n\t"
-#define TOI8_FMA(P)                                                                                   \
-    "mov.b64 zz, {zx" #P ", zy" #P "};\n\t"                                                           \
-    "mov.b64 bb, {pa" #P ", pa" #P "};\n\tmul.rn.f32x2 ta, zz, bb;\n\t"                               \
-    "mov.b64 bb, {pb" #P ", pb" #P "};\n\tmul.rn.f32x2 tb, zz, bb;\n\t"                               \
-    TOI8_ROW("va" #P, "%0", "%8") TOI8_ROW("v1", "%1", "%9") TOI8_ROW("v2", "%2", "%10")              \
-    TOI8_ROW("v3", "%3", "%11") TOI8_ROW("v4", "%4", "%12") TOI8_ROW("v5", "%5", "%13")               \
-    TOI8_ROW("v6", "%6", "%14") TOI8_ROW("v7", "%7", "%15")
-#define TOI8_TEST(K, P, OFF16, OFF32)                                                                 \
-    "ld.shared.v4.b32 {v1, v2, v3, v4}, [%20+" #OFF16 "];\n\t"                                        \
-    "ld.shared.v4.b32 {v5, v6, v7, pad}, [%20+" #OFF32 "];\n\t"                                       \
-    "setp.ne.u32 pq, key" #P ", %17;\n\t"                                                             \
-    "@pq bra S" #K ";\n\t"                                                                            \
-    "B" #K ":\n\t"
-#define TOI8_REC(K, P, PN, OFF16, OFF32, OFFN) TOI8_TEST(K, P, OFF16, OFF32) TOI8_HEAD(PN, OFFN) TOI8_FMA(P)
-#define TOI8_REC_LAST(K, P, OFF16, OFF32) TOI8_TEST(K, P, OFF16, OFF32) TOI8_FMA(P)
-
-// q = &grid[row][col] from 32-bit row / col registers
-#define TOI8_ADDR(ROW, COL)                                                                           \
-    "mul.wide.s32 q, " ROW ", %23;\n\tcvt.s64.s32 q1, " COL ";\n\tadd.s64 q, q, q1;\n\t"             \
-    "shl.b64 q, q, 3;\n\tadd.s64 q, %21, q;\n\t"
-#define TOI8_RED(A) "mov.b64 {x, y}, " A ";\n\tred.global.add.v2.f32 [q], {x, y};\n\t"
-// flush the 8 rows of one column set starting at q (row stride rs64) and clear them
-#define TOI8_FLUSH8(A0, A1, A2, A3, A4, A5, A6, A7)                                                   \
-    TOI8_RED(A0) "add.s64 q, q, rs64;\n\t" TOI8_RED(A1) "add.s64 q, q, rs64;\n\t"                     \
-    TOI8_RED(A2) "add.s64 q, q, rs64;\n\t" TOI8_RED(A3) "add.s64 q, q, rs64;\n\t"                     \
-    TOI8_RED(A4) "add.s64 q, q, rs64;\n\t" TOI8_RED(A5) "add.s64 q, q, rs64;\n\t"                     \
-    TOI8_RED(A6) "add.s64 q, q, rs64;\n\t" TOI8_RED(A7)                                               \
-    "@pz mov.b64 " A0 ", {pad, pad};\n\t@pz mov.b64 " A1 ", {pad, pad};\n\t@pz mov.b64 " A2 ", {pad, pad};\n\t" \
-    "@pz mov.b64 " A3 ", {pad, pad};\n\t@pz mov.b64 " A4 ", {pad, pad};\n\t@pz mov.b64 " A5 ", {pad, pad};\n\t" \
-    "@pz mov.b64 " A6 ", {pad, pad};\n\t@pz mov.b64 " A7 ", {pad, pad};\n\t"
-#define TOI8_SHIFT_DOWN2(A0, A1, A2, A3, A4, A5, A6, A7)                                              \
-    "@pz mul.rn.f32x2 " A0 ", " A2 ", one2;\n\t@pz mul.rn.f32x2 " A1 ", " A3 ", one2;\n\t"             \
-    "@pz mul.rn.f32x2 " A2 ", " A4 ", one2;\n\t@pz mul.rn.f32x2 " A3 ", " A5 ", one2;\n\t"             \
-    "@pz mul.rn.f32x2 " A4 ", " A6 ", one2;\n\t@pz mul.rn.f32x2 " A5 ", " A7 ", one2;\n\t"             \
-    "@pz mov.b64 " A6 ", {pad, pad};\n\t@pz mov.b64 " A7 ", {pad, pad};\n\t"
-#define TOI8_SHIFT_UP2(A0, A1, A2, A3, A4, A5, A6, A7)                                                \
-    "@pz mul.rn.f32x2 " A7 ", " A5 ", one2;\n\t@pz mul.rn.f32x2 " A6 ", " A4 ", one2;\n\t"             \
-    "@pz mul.rn.f32x2 " A5 ", " A3 ", one2;\n\t@pz mul.rn.f32x2 " A4 ", " A2 ", one2;\n\t"             \
-    "@pz mul.rn.f32x2 " A3 ", " A1 ", one2;\n\t@pz mul.rn.f32x2 " A2 ", " A0 ", one2;\n\t"             \
-    "@pz mov.b64 " A0 ", {pad, pad};\n\t@pz mov.b64 " A1 ", {pad, pad};\n\t"
-#define TOI8_SETA "%0", "%1", "%2", "%3", "%4", "%5", "%6", "%7"
-#define TOI8_SETB "%8", "%9", "%10", "%11", "%12", "%13", "%14", "%15"
-#define TOI8_APPLY(M, ...) M(__VA_ARGS__)
-// The window of my group moves to the base cell in key<P> (record K):
-//   * "no sample" record (padding / off-grid): nothing moves;
-//   * near move, (du, dv) each in {-2, 0, 2}: the lanes whose slots hold the two retiring columns
-//     flush those sets (8 cells each) and the slots take the two entering columns; a row move
-//     flushes two cells per set and shifts the rows by two registers;
-//   * first sample of the strip, or a move by more than two cells: every set is flushed and the
-//     window reopens at the new base.
-// Addresses are formed on demand from the packed base cell (no per-lane column pointer is kept).
-#define TOI8_SLOW(K, P, OFF)                                                                          \
-    "S" #K ":\n\t"                                                                                    \
-    "setp.eq.u32 pz, pad, 0;\n\t"                                                                     \
-    "setp.eq.u32 p0, key" #P ", 0x80008000;\n\t"                                                      \
-    "@p0 bra B" #K ";\n\t"                                                                            \
-    "shl.b32 t1, key" #P ", 16;\n\tshr.s32 cu, t1, 16;\n\tshr.s32 cv, key" #P ", 16;\n\t"            \
-    "shl.b32 t1, %17, 16;\n\tshr.s32 ou, t1, 16;\n\tshr.s32 ov, %17, 16;\n\t"                         \
-    "sub.s32 du, cu, ou;\n\tsub.s32 dv, cv, ov;\n\t"                                                  \
-    "add.s32 t1, du, 2;\n\tadd.s32 t2, dv, 2;\n\t"                                                    \
-    "setp.ne.u32 po, %17, 0x80008000;\n\t"                /* window open */                           \
-    "setp.le.and.u32 pn, t1, 4, po;\n\t"                                                              \
-    "setp.le.and.u32 pn, t2, 4, pn;\n\t"                  /* near move */                             \
-    "xor.b32 tpb, %16, 4;\n\t"                            /* window column of my set B */             \
-    "setp.gt.s32 pu, du, 0;\n\t"                                                                      \
-    "selp.s32 t1, 0, 3, pu;\n\t"                          /* retiring column pair: 0,1 or 6,7 */      \
-    "setp.ne.and.s32 pc, du, 0, pn;\n\t"                                                              \
-    "shr.u32 t2, %16, 1;\n\tsetp.eq.and.s32 pfa, t2, t1, pc;\n\t"                                     \
-    "shr.u32 t2, tpb, 1;\n\tsetp.eq.and.s32 pfb, t2, t1, pc;\n\t"                                     \
-    "not.pred pf, pn;\n\tand.pred pf, pf, po;\n\t"        /* far move of an open window: flush all */ \
-    "or.pred pfa, pfa, pf;\n\tor.pred pfb, pfb, pf;\n\t"                                              \
-    "cvt.u64.u32 rs64, %22;\n\t"                                                                      \
-    "@!pfa bra NA" #K ";\n\t"                                                                         \
-    "add.s32 t1, ou, %16;\n\t"                                                                        \
-    TOI8_ADDR("ov", "t1")                                                                             \
-    TOI8_APPLY(TOI8_FLUSH8, TOI8_SETA)                                                                \
-    "NA" #K ":\n\t"                                                                                   \
-    "@!pfb bra NB" #K ";\n\t"                                                                         \
-    "add.s32 t1, ou, tpb;\n\t"                                                                        \
-    TOI8_ADDR("ov", "t1")                                                                             \
-    TOI8_APPLY(TOI8_FLUSH8, TOI8_SETB)                                                                \
-    "NB" #K ":\n\t"                                                                                   \
-    "@!pn bra O" #K ";\n\t"                                                                           \
-    "sub.s32 t1, %16, du;\n\tand.b32 %16, t1, 7;\n\t"     /* my window columns after the column move */ \
-    "xor.b32 tpb, %16, 4;\n\t"                                                                        \
-    "setp.gt.s32 pu, dv, 0;\n\tsetp.lt.s32 pd, dv, 0;\n\t"                                            \
-    "mov.b64 one2, 0x3f8000003f800000;\n\t"                                                           \
-    "add.s32 t1, cu, %16;\n\t"                            /* my set-A column in the new window */     \
-    "sub.s32 t2, tpb, %16;\n\tmul.wide.s32 q2, t2, 8;\n\t" /* set B sits 4 columns right or left */    \
-    "@!pu bra NU" #K ";\n\t"                                                                          \
-    TOI8_ADDR("ov", "t1")                                 /* dv = +2: rows ov, ov + 1 retire */       \
-    TOI8_RED("%0") "add.s64 q, q, q2;\n\t" TOI8_RED("%8")                                             \
-    "sub.s64 q, q, q2;\n\tadd.s64 q, q, rs64;\n\t"                                                    \
-    TOI8_RED("%1") "add.s64 q, q, q2;\n\t" TOI8_RED("%9")                                             \
-    TOI8_APPLY(TOI8_SHIFT_DOWN2, TOI8_SETA)                                                           \
-    TOI8_APPLY(TOI8_SHIFT_DOWN2, TOI8_SETB)                                                           \
-    "NU" #K ":\n\t"                                                                                   \
-    "@!pd bra F" #K ";\n\t"                                                                           \
-    "add.s32 t2, ov, 6;\n\t"                              /* dv = -2: rows ov + 6, ov + 7 retire */   \
-    TOI8_ADDR("t2", "t1")                                                                             \
-    TOI8_RED("%6") "add.s64 q, q, q2;\n\t" TOI8_RED("%14")                                            \
-    "sub.s64 q, q, q2;\n\tadd.s64 q, q, rs64;\n\t"                                                    \
-    TOI8_RED("%7") "add.s64 q, q, q2;\n\t" TOI8_RED("%15")                                            \
-    TOI8_APPLY(TOI8_SHIFT_UP2, TOI8_SETA)                                                             \
-    TOI8_APPLY(TOI8_SHIFT_UP2, TOI8_SETB)                                                             \
-    "bra F" #K ";\n\t"                                                                                \
-    "O" #K ":\n\t"                                                                                    \
-    "sub.s32 t1, %24, cu;\n\tand.b32 %16, t1, 7;\n\t"     /* slot L holds window column (L - bu) mod 8 */ \
-    "xor.b32 tpb, %16, 4;\n\t"                                                                        \
-    "F" #K ":\n\t"                                                                                    \
-    "mov.u32 %17, key" #P ";\n\t"                                                                     \
-    "shl.b32 t1, %16, 2;\n\tadd.u32 t1, t1, 48;\n\tadd.u32 %18, %20, t1;\n\t"                         \
-    "shl.b32 t1, tpb, 2;\n\tadd.u32 t1, t1, 48;\n\tadd.u32 %19, %20, t1;\n\t"                         \
-    "ld.shared.b32 pa" #P ", [%18+" #OFF "];\n\t"                                                     \
-    "ld.shared.b32 pb" #P ", [%19+" #OFF "];\n\t"                                                     \
-    "bra B" #K ";\n\t"
-
-__device__ __forceinline__ void consume_batch(u64 (&a)[kR], u64 (&b)[kR], unsigned &tapA, unsigned &ckey,
-                                              unsigned &rpa, unsigned &rpb, unsigned rgs, const float2 *gc,
-                                              unsigned rs, int G, int L)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .b32 zx0, zy0, key0, va0, pa0, pb0, zx1, zy1, key1, va1, pa1, pb1, pad, v1, v2, v3, v4, v5, v6, v7;\n\t"
-        ".reg .b32 t1, t2, cu, cv, ou, ov, du, dv, tpb;\n\t"
-        ".reg .b64 zz, ta, tb, bb, one2, q, q1, q2, rs64;\n\t"
-        ".reg .f32 x, y;\n\t"
-        ".reg .pred pq, p0, po, pn, pc, pf, pu, pd, pz, pfa, pfb;\n\t"
-        TOI8_HEAD(0, 0)
-        TOI8_REC(0, 0, 1, 16, 32, 80)
-        TOI8_REC(1, 1, 0, 96, 112, 160)
-        TOI8_REC(2, 0, 1, 176, 192, 240)
-        TOI8_REC_LAST(3, 1, 256, 272)
-        "bra DONE;\n\t"
-        TOI8_SLOW(0, 0, 0)
-        TOI8_SLOW(1, 1, 80)
-        TOI8_SLOW(2, 0, 160)
-        TOI8_SLOW(3, 1, 240)
-        "DONE:\n\t"
-        "}"
-        : "+l"(a[0]), "+l"(a[1]), "+l"(a[2]), "+l"(a[3]), "+l"(a[4]), "+l"(a[5]), "+l"(a[6]), "+l"(a[7]),
-          "+l"(b[0]), "+l"(b[1]), "+l"(b[2]), "+l"(b[3]), "+l"(b[4]), "+l"(b[5]), "+l"(b[6]), "+l"(b[7]),
-          "+r"(tapA), "+r"(ckey), "+r"(rpa), "+r"(rpb)
-        : "r"(rgs), "l"(gc), "r"(rs), "r"(G), "r"(L)
-        : "memory");
-}
-
-// Strip end: flush the open window (base cell in ckey): my two column slots, 8 rows each.
-__device__ __forceinline__ void flush_sets(const u64 (&a)[kR], const u64 (&b)[kR], unsigned tapA, unsigned ckey,
-                                           const float2 *gc, long long rs, int G)
-{
-    const int ou = (int)(short)(ckey & 0xffffu), ov = (int)ckey >> 16;
-#pragma unroll
-    for (int set = 0; set < 2; ++set) {
-        const unsigned tap = set ? (tapA ^ 4u) : tapA;
-        const char *p = reinterpret_cast<const char *>(gc + ((long long)ov * G + (ou + (int)tap)));
-#pragma unroll
-        for (int r = 0; r < kR; ++r) {
-            const float2 v = unpack2(set ? b[r] : a[r]);
-            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" : : "l"(p), "f"(v.x), "f"(v.y) : "memory");
-            p += rs;
-        }
-    }
-}
-
-// Raw inputs of one sample as they sit in HBM (requested one batch ahead; decoded at use).
-struct Raw {
-    float2 a, b;      // the two parallel hands
-    float wa, wb;
-    unsigned fl;      // raw flag bytes as loaded (layout depends on MODE); decoded at use
-    double s;         // s_c = nu_c / c0 (not carried when the cell is computed a batch ahead)
-};
-
-// Geometry of one sample, computed one batch AHEAD of its data: the centre cell depends only on the
-// baseline and the channel, so the dependent density lookup of uniform weighting (L2 latency under
-// a streaming load: several hundred cycles) is in flight for a whole batch before it is needed.
-struct Cell {
-    unsigned key;     // packed BASE cell of the sample's window ((centre - 3) & ~1 per axis), kNoKey when off the grid
-    unsigned sh;      // bit 0 / bit 1: the footprint starts at window column / row 1 instead of 0
-    float xu, xv;     // sub-cell offsets
-    float dens;       // D[cell] (1 when there is no density map or the sample is off the grid)
-};
-
-// MODE 4: n_p = 4, hands (0, 3), 16-B aligned weights and 4-B aligned flags -> 2 LDG.64 + LDG.128 + LDG.32
-// MODE 2: n_p = 2, hands (0, 1), 8-B aligned weights, 2-B aligned flags     -> LDG.128 + LDG.64 + LDG.U16
-// MODE 0: anything else, scalar loads
-template <int MODE, bool WITH_S>
-__device__ __forceinline__ void load_raw(const Geometry &g, const Inputs &in, bool has_w, bool has_f,
-                                         long long q, int c, Raw &r)
-{
-    r.s = WITH_S ? __ldg(g.s + c) : 0.0;
-    r.wa = r.wb = 1.0f;
-    r.fl = 0u;
-    if (MODE == 4) {
-        const float2 *v = in.vis + 4 * q;
-        r.a = __ldcs(v);
-        r.b = __ldcs(v + 3);
-        if (has_w) {
-            const float4 w = __ldcs(reinterpret_cast<const float4 *>(in.weights) + q);
-            r.wa = w.x; r.wb = w.w;
-        }
-        if (has_f) r.fl = __ldcs(reinterpret_cast<const unsigned *>(in.flags) + q);
-    } else if (MODE == 2) {
-        const float4 v = __ldcs(reinterpret_cast<const float4 *>(in.vis) + q);
-        r.a = make_float2(v.x, v.y);
-        r.b = make_float2(v.z, v.w);
-        if (has_w) {
-            const float2 w = __ldcs(reinterpret_cast<const float2 *>(in.weights) + q);
-            r.wa = w.x; r.wb = w.y;
-        }
-        if (has_f) r.fl = __ldcs(reinterpret_cast<const unsigned short *>(in.flags) + q);
-    } else {
-        const long long o = q * g.n_p;
-        r.a = __ldcs(in.vis + o + g.pol_a);
-        r.b = __ldcs(in.vis + o + g.pol_b);
-        if (has_w) { r.wa = __ldcs(in.weights + o + g.pol_a); r.wb = __ldcs(in.weights + o + g.pol_b); }
-        if (has_f) r.fl = (unsigned)__ldcs(in.flags + o + g.pol_a) | ((unsigned)__ldcs(in.flags + o + g.pol_b) << 24);
-        if (g.pol_b == g.pol_a) r.fl |= 0xff000000u;     // single hand: b never contributes
-    }
-}
 
 // CHEB: one Chebyshev-moment pass of the near-coplanar mode (struct ChebArgs): only the samples of
 // slab cheb.p contribute, each multiplied by T_k(s_q); never combined with PIPE (the current sample's
@@ -305,11 +63,14 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
     // Chebyshev passes repeat the samples: Wsum / n_gridded once per slab, the rejects once per snapshot
     const bool count = !CHEB || (cheb.count & 1) != 0, count_rej = !CHEB || (cheb.count & 2) != 0;
 
+    // dynamic task queue; the NEXT task is requested while the current one is processed (the atomic's
+    // round trip to L2 was 4 % of the kernel when taken in place)
+    unsigned task_ahead = 0;
+    if (lane == 0) task_ahead = atomicAdd(&st->task_counter, 1u);
     for (;;) {
-        unsigned task = 0;
-        if (lane == 0) task = atomicAdd(&st->task_counter, 1u);
-        task = __shfl_sync(0xffffffffu, task, 0);
+        const unsigned task = __shfl_sync(0xffffffffu, task_ahead, 0);
         if (task >= n_tasks) break;
+        if (lane == 0) task_ahead = atomicAdd(&st->task_counter, 1u);
         const int j = (int)(task / (unsigned)tasks_per_row);
         const int c_task = (int)(task % (unsigned)tasks_per_row) * (kGroups * strip_len);
         double rho1, rho2;
@@ -337,7 +98,8 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                 const int x0 = max(min(iu, ju) - 4 + h, 0) / kTile, x1 = min(max(iu, ju) + 4 + h, G - 1) / kTile;
                 const int y0 = max(min(iv, jv) - 4 + h, 0) / kTile, y1 = min(max(iv, jv) + 4 + h, G - 1) / kTile;
                 for (int ty = y0; ty <= y1; ++ty)
-                    for (int tx = x0; tx <= x1; ++tx) tiles[ty * tpr + tx] = 1;
+                    for (int tx = x0; tx <= x1; ++tx)
+                        if (tiles[ty * tpr + tx] == 0) tiles[ty * tpr + tx] = 1;   // L1 hit instead of a store, mostly
             }
         }
 
@@ -361,21 +123,23 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                 cl.key = cell_key(bu, bv);
                 cl.sh = (unsigned)((iu - kH) & 1) | ((unsigned)((iv - kH) & 1) << 1);
                 if (has_d) cl.dens = __ldg(Dc + ((long long)iv * G + iu));
-            } else if (count_rej) {
-                ++n_off;
+            } else {
+                cl.xu = cl.xv = 0.0f;          // taps stay finite whatever the coordinates were
+                if (count_rej) ++n_off;
             }
         };
-        // software pipeline: raw inputs and cell (+ density) of batch b + 1 are requested while
-        // batch b is processed; the channel scale s_c runs two batches ahead
-        Raw nxt;
-        nxt.a = nxt.b = make_float2(0.0f, 0.0f); nxt.wa = nxt.wb = 0.0f; nxt.fl = 0u; nxt.s = 0.0;
-        Cell cnxt;
-        cnxt.key = kNoKey; cnxt.sh = 0u; cnxt.xu = cnxt.xv = 0.0f; cnxt.dens = 1.0f;
+        // software pipeline: raw inputs and cell (+ density) of batch b + 1 are requested once batch
+        // b's have been used, INTO THE SAME REGISTERS (no current/next copies), and arrive while the
+        // batch is accumulated; the channel scale s_c runs two batches ahead
+        Raw raw;
+        raw.a = raw.b = make_float2(0.0f, 0.0f); raw.wa = raw.wb = 0.0f; raw.fl = 0u; raw.s = 0.0;
+        Cell cell;
+        cell.key = kNoKey; cell.sh = 0u; cell.xu = cell.xv = 0.0f; cell.dens = 1.0f;
         double s_ahead = 0.0;
         if (c_lo < c_hi) {
-            load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c_lo, c_lo, nxt);
+            load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c_lo, c_lo, raw);
             if (PIPE) {
-                locate(__ldg(g.s + c_lo), cnxt);
+                locate(__ldg(g.s + c_lo), cell);
                 if (c_lo + kBatch < c_hi) s_ahead = __ldg(g.s + c_lo + kBatch);
             }
         }
@@ -384,87 +148,82 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
             // ---------------- pre-process one sample per lane ----------------
             {
                 const int c = c_lo + b;
-                const Raw cur = nxt;
-                Cell cell = cnxt;
-                if (c + kBatch < c_hi && b + kBatch < strip_len) {
-                    load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c + kBatch, c + kBatch, nxt);
-                    if (PIPE) {
-                        locate(s_ahead, cnxt);
-                        if (c + 2 * kBatch < c_hi) s_ahead = __ldg(g.s + c + 2 * kBatch);
-                    }
+                const bool live = c < c_hi;
+                if (!PIPE) {
+                    cell.key = kNoKey;
+                    if (live) locate(raw.s, cell);
                 }
-                if (!PIPE && c < c_hi) locate(cur.s, cell);
-                unsigned key = kNoKey;
-                bool valid = false;
-                float wI = 0.0f, zx = 0.0f, zy = 0.0f, pv0 = 0.0f;
-                if (c < c_hi && cell.key != kNoKey) {
-                    // a flagged sample keeps its own cell as key (z = 0, zero taps): it moves the
-                    // window exactly as its unflagged neighbours do and never takes the slow path
-                    key = cell.key;
-                    constexpr unsigned fmask_b = MODE == 2 ? 0x0000ff00u : 0xff000000u;
-                    const float wa = (weight_ok(cur.wa) && !(cur.fl & 0x000000ffu)) ? cur.wa : 0.0f;
-                    const float wb = (weight_ok(cur.wb) && !(cur.fl & fmask_b)) ? cur.wb : 0.0f;
-                    wI = wa + wb;
-                    float tk = 1.0f;
-                    bool mine = true;
-                    if (CHEB && wI > 0.0f) {
-                        // Eq. 19: slab of this sample and its position s_q in it (G24); T_k(s_q) by the
-                        // three-term recurrence in fp64 (T_k amplifies rounding by ~k^2)
-                        const double r3 = __dmul_rn(rho3, cur.s);
-                        int pq = 0;
-                        double sq = 0.0;
-                        if (cheb.d > 0.0) {
-                            pq = min((int)floor((r3 - cheb.r3_min) / (2.0 * cheb.d)), cheb.n_slab - 1);
-                            sq = (r3 - (cheb.r3_min + (2.0 * (double)pq + 1.0) * cheb.d)) / cheb.d;
-                        }
-                        mine = pq == cheb.p;
-                        double t0 = 1.0, t1 = sq;
-                        for (int kk = 1; kk < cheb.k; ++kk) {
-                            const double t2 = fma(2.0 * sq, t1, -t0);
-                            t0 = t1; t1 = t2;
-                        }
-                        tk = (float)(cheb.k == 0 ? 1.0 : t1);
+                // a flagged sample keeps its own cell as key (z = 0): it moves the window exactly as
+                // its unflagged neighbours do and never takes the slow path; the record of a sample
+                // that contributes nothing has z = 0 and finite taps
+                const unsigned key = live ? cell.key : kNoKey;
+                const bool on = key != kNoKey;
+                constexpr unsigned fmask_b = MODE == 2 ? 0x0000ff00u : 0xff000000u;
+                const float wa = (on && weight_ok(raw.wa) && !(raw.fl & 0x000000ffu)) ? raw.wa : 0.0f;
+                const float wb = (on && weight_ok(raw.wb) && !(raw.fl & fmask_b)) ? raw.wb : 0.0f;
+                const float wI = wa + wb;
+                float tk = 1.0f;
+                bool mine = true;
+                if (CHEB && wI > 0.0f) {
+                    // Eq. 19: slab of this sample and its position s_q in it (G24); T_k(s_q) by the
+                    // three-term recurrence in fp64 (T_k amplifies rounding by ~k^2)
+                    const double r3 = __dmul_rn(rho3, raw.s);
+                    int pq = 0;
+                    double sq = 0.0;
+                    if (cheb.d > 0.0) {
+                        pq = min((int)floor((r3 - cheb.r3_min) / (2.0 * cheb.d)), cheb.n_slab - 1);
+                        sq = (r3 - (cheb.r3_min + (2.0 * (double)pq + 1.0) * cheb.d)) / cheb.d;
                     }
-                    if (!(wI > 0.0f)) {
-                        if (count_rej) ++n_flag;
-                    } else if (mine) {
-                        if (count) ++n_grid;
-                        valid = true;
-                        // z = w_a Vis_a + w_b Vis_b; a zero-weight hand is skipped (its data may be NaN)
-                        if (wa > 0.0f) { zx = wa * cur.a.x; zy = wa * cur.a.y; }
-                        if (wb > 0.0f) { zx = fmaf(wb, cur.b.x, zx); zy = fmaf(wb, cur.b.y, zy); }
-                        if (CHEB) { zx *= tk; zy *= tk; }
-                        float pu[kW], pv[kW];
-                        kernel_taps2(cell.xu, cell.xv, pu, pv);
-                        // the 7 taps sit at window offset 0 or 1 on each axis; the free end is zero
-                        const bool su = (cell.sh & 1u) != 0u, sv = (cell.sh & 2u) != 0u;
-                        unsigned wu[kR], wv[kR];
-#pragma unroll
-                        for (int i = 0; i < kR; ++i) {
-                            const float lo_u = i < kW ? pu[i] : 0.0f, hi_u = i > 0 ? pu[i - 1] : 0.0f;
-                            const float lo_v = i < kW ? pv[i] : 0.0f, hi_v = i > 0 ? pv[i - 1] : 0.0f;
-                            wu[i] = __float_as_uint(su ? hi_u : lo_u);
-                            wv[i] = __float_as_uint(sv ? hi_v : lo_v);
-                        }
-                        pv0 = __uint_as_float(wv[0]);
-                        my_rec[1] = make_uint4(wv[1], wv[2], wv[3], wv[4]);
-                        my_rec[2] = make_uint4(wv[5], wv[6], wv[7], 0u);
-                        my_rec[3] = make_uint4(wu[0], wu[1], wu[2], wu[3]);
-                        my_rec[4] = make_uint4(wu[4], wu[5], wu[6], wu[7]);
+                    mine = pq == cheb.p;
+                    double t0 = 1.0, t1 = sq;
+                    for (int kk = 1; kk < cheb.k; ++kk) {
+                        const double t2 = fma(2.0 * sq, t1, -t0);
+                        t0 = t1; t1 = t2;
                     }
+                    tk = (float)(cheb.k == 0 ? 1.0 : t1);
                 }
-                if (!valid) {
-                    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
-                    my_rec[1] = zero; my_rec[2] = zero; my_rec[3] = zero; my_rec[4] = zero;
-                }
+                const bool valid = wI > 0.0f && mine;
+                if (on && !(wI > 0.0f) && count_rej) ++n_flag;
+                if (valid && count) ++n_grid;
+                // z = w_a Vis_a + w_b Vis_b; a zero-weight hand is skipped (its data may be NaN)
+                float zx = 0.0f, zy = 0.0f;
+                if (wa > 0.0f) { zx = wa * raw.a.x; zy = wa * raw.a.y; }
+                if (wb > 0.0f) { zx = fmaf(wb, raw.b.x, zx); zy = fmaf(wb, raw.b.y, zy); }
+                if (CHEB) { zx *= tk; zy *= tk; }
+                if (!valid) zx = zy = 0.0f;
                 float f = 1.0f;
                 if (has_d) {
                     // the density of a cell whose samples are all flagged is 0: never invert it
                     const float dens = valid ? cell.dens : 1.0f;
                     asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(f) : "f"(dens));
                 }
-                if (!CHEB || (count && valid)) wpart = fmaf(f, wI, wpart);
-                my_rec[0] = make_uint4(__float_as_uint(zx * f), __float_as_uint(zy * f), key, __float_as_uint(pv0));
+                if (!CHEB || count) wpart = fmaf(f, valid ? wI : 0.0f, wpart);
+                const float xu = cell.xu, xv = cell.xv;
+                const bool su = (cell.sh & 1u) != 0u, sv = (cell.sh & 2u) != 0u;
+                // ---- this batch's raw inputs and cell are used up: request the next batch's ----
+                if (c + kBatch < c_hi && b + kBatch < strip_len) {
+                    load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c + kBatch, c + kBatch, raw);
+                    if (PIPE) {
+                        locate(s_ahead, cell);
+                        if (c + 2 * kBatch < c_hi) s_ahead = __ldg(g.s + c + 2 * kBatch);
+                    }
+                }
+                float pu[kW], pv[kW];
+                kernel_taps2(xu, xv, pu, pv);
+                // the 7 taps sit at window offset 0 or 1 on each axis; the free end is zero
+                unsigned wu[kR], wv[kR];
+#pragma unroll
+                for (int i = 0; i < kR; ++i) {
+                    const float lo_u = i < kW ? pu[i] : 0.0f, hi_u = i > 0 ? pu[i - 1] : 0.0f;
+                    const float lo_v = i < kW ? pv[i] : 0.0f, hi_v = i > 0 ? pv[i - 1] : 0.0f;
+                    wu[i] = __float_as_uint(su ? hi_u : lo_u);
+                    wv[i] = __float_as_uint(sv ? hi_v : lo_v);
+                }
+                my_rec[1] = make_uint4(wv[1], wv[2], wv[3], wv[4]);
+                my_rec[2] = make_uint4(wv[5], wv[6], wv[7], 0u);
+                my_rec[3] = make_uint4(wu[0], wu[1], wu[2], wu[3]);
+                my_rec[4] = make_uint4(wu[4], wu[5], wu[6], wu[7]);
+                my_rec[0] = make_uint4(__float_as_uint(zx * f), __float_as_uint(zy * f), key, wv[0]);
             }
             __syncwarp();
             // ---------------- accumulate: every group consumes its 4 records ----------------

@@ -283,10 +283,12 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     }
     CU_TRY(p, cudaEventRecord(p->ev[EV_WEIGHT], stream));
     // a3 + a5: cell indices and gridding onto the zero grid
-    const bool sliding = p->cfg.gridder == TOI_GRIDDER_SLIDING;
+    const bool sliding = p->cfg.gridder != TOI_GRIDDER_ATOMIC;
     uint8_t *tiles = gridder_tile_map(p, stream, sliding);
-    if (sliding)
+    if (p->cfg.gridder == TOI_GRIDDER_SLIDING)
         launch_grid_pair8(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
+    else if (p->cfg.gridder == TOI_GRIDDER_WS)
+        launch_grid_ws(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
     else
         launch_grid_atomic(g, in, p->d_state, dens, p->d_grid, stream);
     launches += tiles ? 1 : 2;
@@ -386,7 +388,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     if (W != kW) return fail(nullptr, TOI_ERR_UNSUPPORTED, "only kernel_support = 7 is built");
     if (cfg->weighting != TOI_WEIGHT_NATURAL && cfg->weighting != TOI_WEIGHT_UNIFORM) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown weighting");
     if (cfg->input_location != TOI_MEM_HOST && cfg->input_location != TOI_MEM_DEVICE) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown input_location");
-    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC)
+    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC && cfg->gridder != TOI_GRIDDER_WS)
         return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown gridder");
     if ((cfg->enable_3d != 0 && cfg->enable_3d != 1) || (cfg->debug_keep_grid != 0 && cfg->debug_keep_grid != 1))
         return fail(nullptr, TOI_ERR_INVALID_ARG, "enable_3d and debug_keep_grid must be 0 or 1");
@@ -655,7 +657,7 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     if (!uvw_m || !vis || !d_image_out) return fail(p, TOI_ERR_INVALID_ARG, "uvw_m, vis and d_image_out must be non-NULL");
     if (n_slab_in < 0 || n_slab_in > 1024 || K_in < 0 || K_in > 64) return fail(p, TOI_ERR_INVALID_ARG, "n_slab must be in [0, 1024], K in [0, 64]");
     if (!p->d_acc3) return fail(p, TOI_ERR_UNSUPPORTED, "the 3-D mode needs a plan created with enable_3d = 1");
-    if (p->cfg.gridder != TOI_GRIDDER_SLIDING) return fail(p, TOI_ERR_UNSUPPORTED, "the 3-D mode runs on the sliding gridder only");
+    if (p->cfg.gridder == TOI_GRIDDER_ATOMIC) return fail(p, TOI_ERR_UNSUPPORTED, "the 3-D mode runs on the sliding gridders only");
     const Geometry &g = p->geo;
     CU_TRY(p, cudaSetDevice(p->cfg.device));
     cudaStream_t stream = cuda_stream ? (cudaStream_t)cuda_stream : p->s_compute;
@@ -733,7 +735,10 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
             const bool last = sp == slabs_run - 1 && k == K - 1;
             CU_TRY(p, cudaMemsetAsync(&p->d_state->task_counter, 0, sizeof(unsigned int), stream));
             uint8_t *tiles = gridder_tile_map(p, stream, true);
-            launch_grid_pair8_cheb(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, ca, stream);
+            if (p->cfg.gridder == TOI_GRIDDER_WS)
+                launch_grid_ws_cheb(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, ca, stream);
+            else
+                launch_grid_pair8_cheb(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, ca, stream);
             launches += tiles ? 2 : 3;
             if (first && p->keep_grid) {
                 CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));

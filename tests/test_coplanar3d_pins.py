@@ -110,3 +110,27 @@ def test_C5_chebyshev_image_equals_the_direct_3d_sum(n_slab, K):
     # and the r3 term matters here: dropping it (the 2-D approximation, Eq. 7) is far off
     flat = o3.image_3d_direct(np.column_stack([r[:, 0], r[:, 1], np.zeros(n)]), vis, V, omega, N, cell)
     assert np.max(np.abs(flat[ok] - direct[ok])) > 100 * np.max(np.abs(cheb[ok] - direct[ok]))
+
+
+def test_C6_pixel_list_form_of_eq18_equals_the_full_image_form():
+    """image_3d_direct_pixels (used where the full N x N sum is too large) is the same Eq. 18 sum as
+    image_3d_direct, pixel by pixel -- including the NaN outside the sphere constraint and the
+    chunking over samples."""
+    rng = np.random.default_rng(11)
+    t = math.radians(50.0)
+    V = minimal_rotation(math.sin(t) * 0.8, -math.sin(t) * 0.6)
+    n, N, cell = 45, 20, 3.0                                    # 60 deg field: some pixels leave the sphere
+    r = np.column_stack([rng.normal(0, 10, n), rng.normal(0, 10, n), rng.normal(0, 3.0, n)])
+    vis = rng.normal(size=n) + 1j * rng.normal(size=n)
+    omega = abs(V[0, 0] * V[1, 1] - V[1, 0] * V[0, 1])
+    full = o3.image_3d_direct(r, vis, V, omega, N, cell, wsum=17.5)
+    jj, ii = np.mgrid[0:N, 0:N]
+    got = o3.image_3d_direct_pixels(r, vis, V, omega, N, cell, ii.ravel(), jj.ravel(), wsum=17.5, chunk=7).reshape(N, N)
+    assert np.isnan(full).any() and not np.isnan(full).all()
+    assert np.array_equal(np.isnan(got), np.isnan(full))
+    ok = ~np.isnan(full)
+    assert np.max(np.abs(got[ok] - full[ok])) <= 1e-12 * np.max(np.abs(full[ok]))
+    # transposed pixel arguments would show: the image is not symmetric
+    swapped = o3.image_3d_direct_pixels(r, vis, V, omega, N, cell, jj.ravel(), ii.ravel(), wsum=17.5).reshape(N, N)
+    both = ok & ~np.isnan(swapped)
+    assert np.max(np.abs(swapped[both] - full[both])) > 1e-3 * np.max(np.abs(full[ok]))

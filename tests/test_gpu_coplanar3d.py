@@ -91,6 +91,9 @@ def test_3d_mode_matches_the_chebyshev_oracle(n_slab, K, flags):
     wsum = float(np.sum(wI))
     img3, i3, info, img2 = run_gpu(snap, N, cell, n_slab, K)
     assert info["n_off_grid"] == 0 and info["n_gridded"] == z.size        # every sample on the grid, counted once
+    n_flagged = 0 if snap["flags"] is None else int(np.count_nonzero(np.all(snap["flags"] != 0, axis=2)))
+    assert info["n_flagged"] == n_flagged                                   # ... also with several slabs
+    assert not flags or n_flagged > 0
     assert abs(info["wsum"] - wsum) <= 2e-6 * wsum
     assert np.max(np.abs(np.array(info["V"]) - V)) < 1e-12
     assert i3["n_slab"] == n_slab and i3["K"] == K and i3["n_passes"] == n_slab * K
@@ -193,3 +196,127 @@ def test_3d_mode_with_host_inputs_equals_device_inputs_and_refuses_bad_arguments
         assert lib.toi_image_snapshot_3d(plan, None, args[1], None, None, None, 1, 8, C.byref(out), None, None) == toi.TOI_ERR_INVALID_ARG
     finally:
         toi.toi_plan_destroy(plan)
+
+
+@pytest.mark.parametrize("weighting", [toi.TOI_WEIGHT_NATURAL, toi.TOI_WEIGHT_UNIFORM])
+@pytest.mark.parametrize("order", [("2d", "3d", "2d"), ("3d", "2d", "2d"), ("2d", "3d", "3d", "3d", "2d", "3d")])
+def test_2d_and_3d_calls_in_any_order_share_one_clean_grid(weighting, order):
+    """2-D and 3-D calls alternate on one plan in every parity: the single gridding grid (and density
+    map) must be zero again after each call, whichever mode ran last.  Planar array => both modes give
+    the same image."""
+    planar = make_snapshot(seed=21, bump_m=0.0, flags=True)
+    N, cell = 64, 200.0 / 3600.0
+    n_b, n_c, n_p = planar["vis"].shape
+    plan = toi.toi_plan_create(n_b, n_c, n_p, planar["chan_freq_hz"], N, cell, weighting=weighting,
+                               input_location=toi.TOI_MEM_DEVICE, enable_3d=True)
+    try:
+        t = {k: (None if planar[k] is None else torch.from_numpy(np.ascontiguousarray(planar[k])).cuda())
+             for k in ("uvw_m", "vis", "weights", "flags")}
+        ptr, info0, _ = toi.toi_image_snapshot(plan, t["uvw_m"], t["vis"], t["weights"], t["flags"], want_info=True)
+        ref = toi.toi_copy_image_to_host(plan, ptr, N).numpy().copy()
+        peak = float(np.max(np.abs(ref)))
+        for kind in order:
+            if kind == "2d":
+                ptr, info, _ = toi.toi_image_snapshot(plan, t["uvw_m"], t["vis"], t["weights"], t["flags"], want_info=True)
+            else:
+                ptr, _, info = toi.toi_image_snapshot_3d(plan, t["uvw_m"], t["vis"], t["weights"], t["flags"])
+            img = toi.toi_copy_image_to_host(plan, ptr, N).numpy()
+            ok = ~np.isnan(img)
+            assert ok.mean() > 0.9
+            assert np.max(np.abs(img[ok] - ref[ok])) <= 1e-5 * peak, (kind, order)
+            assert info.n_gridded == info0.n_gridded and info.n_flagged == info0.n_flagged
+    finally:
+        toi.toi_plan_destroy(plan)
+
+
+def test_stream_after_one_3d_call():
+    """toi_image_stream started after a single 3-D call (host-input plan): same images as before it."""
+    import ctypes as C
+    snap = make_snapshot(seed=23, bump_m=0.0)
+    N, cell = 64, 200.0 / 3600.0
+    n_b, n_c, n_p = snap["vis"].shape
+    plan = toi.toi_plan_create(n_b, n_c, n_p, snap["chan_freq_hz"], N, cell, input_location=toi.TOI_MEM_HOST,
+                               enable_3d=True, image_ring_depth=4)
+    try:
+        t = {k: (None if snap[k] is None else torch.from_numpy(np.ascontiguousarray(snap[k])).pin_memory())
+             for k in ("uvw_m", "vis", "weights", "flags")}
+        ptr, _, _ = toi.toi_image_snapshot(plan, t["uvw_m"], t["vis"], t["weights"], t["flags"], want_info=True)
+        ref = toi.toi_copy_image_to_host(plan, ptr, N).numpy().copy()
+        toi.toi_image_snapshot_3d(plan, t["uvw_m"], t["vis"], t["weights"], t["flags"])
+        got = {}
+
+        def fill(idx, slot):
+            for name, dst in (("uvw_m", slot.uvw_m), ("vis", slot.vis), ("weights", slot.weights)):
+                a = np.ascontiguousarray(snap[name])
+                C.memmove(dst, a.ctypes.data, a.nbytes)
+            slot.flags = None
+            return 0
+
+        def sink(idx, d_image, stream, info):
+            got[idx] = d_image
+
+        toi.toi_image_stream(plan, 3, fill, sink)
+        for k in range(3):
+            img = toi.toi_copy_image_to_host(plan, got[k], N).numpy()
+            assert np.max(np.abs(img - ref)) <= 2e-6 * float(np.max(np.abs(ref)))
+    finally:
+        toi.toi_plan_destroy(plan)
+
+
+@pytest.mark.slow
+def test_3d_mode_at_config5_full_size_against_eq18():
+    """BASELINE.json configs[4] at full size (2016 baselines x 1024 channels x 4 pols, N = 4096,
+    G = 8192, low elevation): the instantiation bench.py times (4 pols, automatic N_slab and K) against
+    Eq. 18 ITSELF at sampled pixels -- centre, brightest 2-D pixel, the four corners, seeded others.
+    Bound: 1.5 x the sampled expansion error + 2e-5, times sum|z| / Wsum (the gridding + fp32 share)."""
+    from paper_2512_06254_b200 import synth
+    wl = synth.CONFIG5
+    dev = synth.make_snapshot(wl, 0, device="cuda")
+    snap = {k: (v.cpu().numpy() if v is not None else None) for k, v in dev.items()}
+    N, cell = wl.image_size, wl.cell_size_deg
+    plan = toi.toi_plan_create(wl.n_baselines, wl.n_chan, wl.n_pol, snap["chan_freq_hz"], N, cell, pol_a=0, pol_b=3,
+                               input_location=toi.TOI_MEM_DEVICE, enable_3d=True)
+    try:
+        ptr, i3, info = toi.toi_image_snapshot_3d(plan, dev["uvw_m"], dev["vis"], dev["weights"], dev["flags"])
+        img3 = toi.toi_copy_image_to_host(plan, ptr, N).numpy().copy()
+        ptr2, _, _ = toi.toi_image_snapshot(plan, dev["uvw_m"], dev["vis"], dev["weights"], dev["flags"], want_info=True)
+        img2 = toi.toi_copy_image_to_host(plan, ptr2, N).numpy().copy()
+    finally:
+        toi.toi_plan_destroy(plan)
+    del dev
+    torch.cuda.empty_cache()
+    rc, V, omega, _ = oracle.plane_fit(snap["uvw_m"], snap["chan_freq_hz"])
+    assert rc == 0 and np.max(np.abs(np.array(info.as_dict()["V"]) - V)) < 1e-12
+    # the samples the gridder keeps: on the grid (G10) and not flagged; hands 0 and 3
+    rho = oracle.rotate(snap["uvw_m"], V)
+    _, _, on = oracle.cell_indices(rho, snap["chan_freq_hz"], 2 * N, cell)
+    s = snap["chan_freq_hz"] / C0
+    w = snap["weights"][:, :, [0, 3]].astype(np.float64)
+    w = np.where(snap["flags"][:, :, [0, 3]] != 0, 0.0, w)
+    z = np.sum(w * snap["vis"][:, :, [0, 3]].astype(np.complex128), axis=2)
+    wI = np.sum(w, axis=2)
+    keep = (wI > 0) & on
+    r = (rho[:, None, :] * s[None, :, None])[keep]
+    z, wI = z[keep], wI[keep]
+    wsum = float(np.sum(wI))
+    assert info.n_gridded == z.size and abs(info.wsum - wsum) <= 2e-6 * wsum
+    phi_o, _ = o3.phi_max_of(V, r[:, 2], N, cell)
+    want = o3.select_parameters(phi_o)
+    assert i3["n_slab"] == want["n_slab"] and i3["K"] == want["K"] and i3["n_passes"] == want["n_slab"] * want["K"]
+    rng = np.random.default_rng(55)
+    jj, ii = np.unravel_index(np.nanargmax(img2), img2.shape)
+    pi = np.concatenate([[N // 2, ii, 0, N - 1, 0, N - 1], rng.integers(0, N, 6)])
+    pj = np.concatenate([[N // 2, jj, 0, 0, N - 1, N - 1], rng.integers(0, N, 6)])
+    direct = o3.image_3d_direct_pixels(r, z, V, omega, N, cell, pi, pj, wsum=wsum)
+    got = img3[pj, pi]
+    assert np.array_equal(np.isnan(got), np.isnan(direct.real))
+    ok = ~np.isnan(got)
+    assert ok.sum() >= 8
+    scale = float(np.sum(np.abs(z))) / wsum
+    eps = o3.sampled_error(phi_o / i3["n_slab"], i3["K"])
+    err = float(np.max(np.abs(got[ok] - direct.real[ok])))
+    err2d = float(np.max(np.abs(img2[pj, pi][ok] - direct.real[ok])))
+    print("3-D mode, config 5 full size: n_slab %d K %d phi_max %.2f; max |err| vs Eq. 18 = %.3e = %.3e x scale "
+          "(sampled expansion error %.3e); the 2-D image is off by %.3e" %
+          (i3["n_slab"], i3["K"], phi_o, err, err / scale, eps, err2d))
+    assert err <= (1.5 * eps + 2e-5) * scale

@@ -92,7 +92,7 @@ def _check_all(snap, wl_N, cell, weighting, gridder, pol_a=None, pol_b=None, loc
 # ------------------------------------------------------------------------------------------------
 # config 1 (BASELINE.json configs[0]): the tiny snapshot, natural weighting, both gridders
 # ------------------------------------------------------------------------------------------------
-ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_ATOMIC]
+ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_WS, toi.TOI_GRIDDER_ATOMIC]
 
 
 @pytest.mark.parametrize("gridder", ALL_GRIDDERS)
@@ -489,3 +489,119 @@ def test_configs_4_and_5_full_size(cfg, n_dft):
     assert rc == 0
     peak = float(np.max(np.abs(img_o)))
     assert np.max(np.abs(img_g[pj, pi] - re)) <= MAX_ABS_BAR * peak
+
+
+# ------------------------------------------------------------------------------------------------
+# the sparse clear (k_clear.cu): tiles marked by the gridder / the density pass, or all of them
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("weighting", ["natural", "uniform"])
+def test_unsorted_channels_take_the_mark_every_tile_path(weighting):
+    """The gridder bounds the tiles a strip can touch by the strip's two end samples, which needs
+    monotone channel frequencies; a plan with shuffled channels marks every tile instead.  Same image
+    as the oracle (which does not care about the channel order), twice in a row, and the same again
+    after a DIFFERENT snapshot was imaged in between (nothing of it may be left on the grid)."""
+    wl = _reduced2(n_ant=14, n_chan=200, image_size=256)
+    snap = snapshot_np(wl)
+    other = snapshot_np(wl, 7)
+    perm = np.random.default_rng(5).permutation(wl.n_chan)
+    for s in (snap, other):
+        s["chan_freq_hz"] = np.ascontiguousarray(s["chan_freq_hz"][perm])
+        for k in ("vis", "weights", "flags"):
+            s[k] = np.ascontiguousarray(s[k][:, perm, :])
+    rc, img_o, info_o, _ = _oracle(snap, wl.image_size, wl.cell_size_deg, weighting, pol_a=0, pol_b=3)
+    assert rc == 0
+    with GpuImager(snap, wl.image_size, wl.cell_size_deg, weighting, pol_a=0, pol_b=3) as gi:
+        for k in range(4):
+            gi.set_inputs(other if k == 2 else snap)
+            img, info, _ = gi.image()
+            if k != 2:
+                assert info["n_gridded"] == info_o["n_gridded"]
+                _assert_image(img, img_o, "shuffled channels, call %d" % k)
+
+
+@pytest.mark.parametrize("weighting", ["natural", "uniform"])
+def test_different_snapshots_in_a_row_leave_nothing_behind(weighting):
+    """Sparse clear with the gridder's own tile marks (sorted channels): snapshots with different
+    geometry (hour angles 20 min apart: other tiles) alternate on one plan; each image equals its oracle."""
+    wl = synth.reduced(_reduced2(n_ant=14, n_chan=160, image_size=256), dt_s=1200.0)
+    snaps = [snapshot_np(wl, k) for k in range(3)]
+    refs = [_oracle(s, wl.image_size, wl.cell_size_deg, weighting, pol_a=0, pol_b=3)[1] for s in snaps]
+    with GpuImager(snaps[0], wl.image_size, wl.cell_size_deg, weighting, pol_a=0, pol_b=3) as gi:
+        for k in (0, 1, 2, 0, 2, 1):
+            gi.set_inputs(snaps[k])
+            img, _, _ = gi.image()
+            _assert_image(img, refs[k], "snapshot %d" % k)
+
+
+def test_debug_exports_need_their_plan_flag():
+    wl = synth.reduced(synth.CONFIG1, n_ant=6, n_core=6, n_chan=8, image_size=32, cell_arcsec=60.0)
+    snap = snapshot_np(wl)
+    with GpuImager(snap, wl.image_size, wl.cell_size_deg) as gi:
+        with pytest.raises(toi.ToiError) as ei:
+            toi.toi_debug_keep_grid(gi.plan, True)
+        assert ei.value.code == toi.TOI_ERR_UNSUPPORTED
+        with pytest.raises(toi.ToiError) as ei:
+            toi.toi_image_snapshot_3d(gi.plan, gi.t["uvw_m"], gi.t["vis"])
+        assert ei.value.code == toi.TOI_ERR_UNSUPPORTED
+    with pytest.raises(toi.ToiError) as ei:            # G > 32768: a window base must fit 2 x 16 bits
+        toi.toi_plan_create(3, 2, 2, [1.0e9, 1.1e9], 64, 0.01, grid_size=32770)
+    assert ei.value.code == toi.TOI_ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------------
+# full size: the other configs of BASELINE.json, at the sizes bench.py times
+# ------------------------------------------------------------------------------------------------
+def _full_size_case(wl, snapshot, weighting, n_dft, what):
+    dev = synth.make_snapshot(wl, snapshot, device="cuda")
+    snap = {k: (v.cpu().numpy() if v is not None else None) for k, v in dev.items()}
+    del dev
+    torch.cuda.empty_cache()
+    N, cell = wl.image_size, wl.cell_size_deg
+    rc, img_o, info_o, _ = _oracle(snap, N, cell, weighting, pol_a=0, pol_b=3)
+    assert rc == 0
+    with GpuImager(snap, N, cell, weighting, pol_a=0, pol_b=3) as gi:
+        img_g, info_g, _ = gi.image()
+    assert np.max(np.abs(np.array(info_g["V"]) - info_o["V"])) <= 1e-12
+    for k in ("n_gridded", "n_off_grid", "n_flagged"):
+        assert abs(info_g[k] - info_o[k]) <= max(2, info_o["n_gridded"] // 100000), k    # own V on both sides (G5 iii)
+    assert abs(info_g["wsum"] - info_o["wsum"]) <= 2e-6 * abs(info_o["wsum"])
+    e = _assert_image(img_g, img_o, what)
+    print("%s: rel-L2 %.3e, max/peak %.3e" % (what, e[0], e[1]))
+    if n_dft:
+        rng = np.random.default_rng(wl.config_id + snapshot)
+        jj, ii = np.unravel_index(np.argmax(img_o), img_o.shape)
+        pi = np.concatenate([[N // 2, ii], rng.integers(0, N, n_dft - 2)]).astype(np.int32)
+        pj = np.concatenate([[N // 2, jj], rng.integers(0, N, n_dft - 2)]).astype(np.int32)
+        wt = oracle.UNIFORM if weighting == "uniform" else oracle.NATURAL
+        rc, re, _, _ = oracle.image_dft_pixels(snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"],
+                                               snap["chan_freq_hz"], N, cell, pi, pj, weighting=wt, pol_a=0, pol_b=3)
+        assert rc == 0
+        peak = float(np.max(np.abs(img_o)))
+        assert np.max(np.abs(img_g[pj, pi] - re)) <= MAX_ABS_BAR * peak
+    return snap, img_g, info_o
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("snapshot", [0, 749, 1499])
+def test_config3_stream_snapshots_full_size(snapshot):
+    """BASELINE.json configs[2]: snapshots 0, 749 and 1499 of the 1500-snapshot run (hour angle advanced
+    by 0, 25 and 50 minutes; the 5 mJy pulsar is off, ON, off), uniform weighting, against Tier G."""
+    wl = synth.CONFIG3
+    l, m, flux = synth.sky_model(wl, snapshot)
+    assert (float(flux[-1]) > 0.0) == (snapshot == 749)
+    _full_size_case(wl, snapshot, "uniform", 0, "config 3 snapshot %d uniform" % snapshot)
+
+
+@pytest.mark.slow
+def test_config4_uniform_full_size():
+    """BASELINE.json configs[3] asks for natural AND uniform: the uniform half (density pass over 66 M
+    samples, 1 GB density map), whole image against Tier G plus sampled pixels against Tier D."""
+    _full_size_case(synth.CONFIG4, 0, "uniform", 4, "config 4 uniform")
+
+
+@pytest.mark.slow
+def test_config5_last_snapshot_full_size():
+    """BASELINE.json configs[4]: the other end of the elevation sweep (snapshot 511, elevation 35 deg,
+    plane tilt ~55 deg; snapshot 0 at 20 deg / 70 deg is test_configs_4_and_5_full_size)."""
+    snap, _, info_o = _full_size_case(synth.CONFIG5, 511, "natural", 6, "config 5 snapshot 511")
+    assert 0.5 < info_o["omega"] < 0.65

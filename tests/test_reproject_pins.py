@@ -131,6 +131,33 @@ def test_R6_bilinear_gather_matches_scipy():
     assert np.max(np.abs(out[inside] - ref[inside])) < 1e-12
 
 
+def test_R8_edge_rule_of_reading_G22():
+    """DESIGN.md G22: a position within 1e-6 px outside [0, N-1]^2 counts as on the edge (and is clipped
+    to it), anything further out is NaN.  (a) With V = I the map must be the identity INCLUDING the
+    last row and column, whatever the rounding: for N = 250 and this cell size the fp64 evaluation of
+    Eq. 16 puts the last column 1.4e-14 px outside -- without the tolerance that column would be lost;
+    (b) a position 5e-7 px outside takes the edge value, one 1e-5 px outside is NaN -- a tolerance of
+    1e-3 would keep it."""
+    N, cell = 250, 0.1061373992010266
+    p1, p2, ok = orp.map_exact(np.eye(3), N, cell)
+    over = max(p1.max() - (N - 1), -p1.min(), p2.max() - (N - 1), -p2.min())
+    assert 0.0 < over < 1e-12                                   # the rounding this rule exists for
+    rng = np.random.default_rng(4)
+    img = rng.normal(size=(N, N))
+    out = orp.reproject(img, np.eye(3), cell, "exact")
+    assert not np.isnan(out).any()
+    assert np.max(np.abs(out - img)) < 1e-9
+    M = 8
+    small = rng.normal(size=(M, M))
+    p1 = np.full((1, 6), 3.0)
+    p2 = np.full((1, 6), 2.0)
+    p1[0, :] = [M - 1 + 5e-7, M - 1 + 1e-5, -5e-7, -1e-5, 3.0, 3.0]
+    p2[0, 4:] = [M - 1 + 5e-7, -1e-5]
+    got = orp.bilinear_gather(small, p1, p2, np.ones((1, 6), bool))[0]
+    assert got[0] == small[2, M - 1] and got[2] == small[2, 0] and abs(got[4] - small[M - 1, 3]) < 1e-15
+    assert np.isnan(got[1]) and np.isnan(got[3]) and np.isnan(got[5])
+
+
 def test_R6_bilinear_reproduces_affine_images_exactly():
     N = 32
     jj, ii = np.mgrid[0:N, 0:N].astype(np.float64)
