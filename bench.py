@@ -45,7 +45,7 @@ def parse_args():
     ap.add_argument("--workload", type=int, default=2, choices=[1, 2, 4, 5],
                     help="BASELINE.json config id (2 = configs[1], the metric's workload)")
     ap.add_argument("--weighting", default=None, choices=[None, "natural", "uniform"])
-    ap.add_argument("--gridder", default="sliding", choices=["sliding", "atomic", "ws"])
+    ap.add_argument("--gridder", default="sliding", choices=["sliding", "atomic", "ws", "tma"])
     ap.add_argument("--stream-snapshots", type=int, default=1500,
                     help="length of the streamed (configs[2]) run reported under `stream`; 0 = skip")
     ap.add_argument("--stream-pool", type=int, default=16,
@@ -297,7 +297,7 @@ def run_ours(args):
     toi.load()
     wl, weighting = workload(args)
     wt = toi.TOI_WEIGHT_UNIFORM if weighting == "uniform" else toi.TOI_WEIGHT_NATURAL
-    gridder = {"sliding": toi.TOI_GRIDDER_SLIDING, "atomic": toi.TOI_GRIDDER_ATOMIC, "ws": toi.TOI_GRIDDER_WS}[args.gridder]
+    gridder = {"sliding": toi.TOI_GRIDDER_SLIDING, "atomic": toi.TOI_GRIDDER_ATOMIC, "ws": toi.TOI_GRIDDER_WS, "tma": toi.TOI_GRIDDER_TMA}[args.gridder]
     S = wl.n_baselines * wl.n_chan
     N = wl.image_size
     snap = make_inputs(wl, "cuda")            # seeded generator, on the device; every rank the same shape
@@ -521,7 +521,7 @@ def main():
         return
     ab = algorithmic_bytes(wl, weighting)
     peak, peak_src = measured_peaks()
-    kernel = {"sliding": "k_grid_pair8", "atomic": "k_grid_atomic", "ws": "k_grid_ws"}[args.gridder]
+    kernel = {"sliding": "k_grid_pair8", "atomic": "k_grid_atomic", "ws": "k_grid_ws", "tma": "k_grid_tma"}[args.gridder]
     roofline = roofline_of(wl, weighting, r["stages"], r["stages_min"], peak, peak_src, kernel)
     tr = NCU_TRAFFIC.get((str(args.workload), weighting, args.gridder))
     roofline["traffic"] = None if tr is None else tr["bytes"]

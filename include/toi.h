@@ -53,7 +53,7 @@ enum { TOI_MEM_HOST = 0, TOI_MEM_DEVICE = 1 };
  * float atomics, k_grid_atomic.cu) is the ncu comparison point the design replaces and a second,
  * structurally different implementation for the parity tests.  Both give the same image within
  * the parity bars. */
-enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1, TOI_GRIDDER_WS = 2 };
+enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1, TOI_GRIDDER_WS = 2, TOI_GRIDDER_TMA = 3 };
 
 /* The paper's inputs (Measurement Set, image size, cell size) plus the knobs the
  * paper leaves open.  Zero selects the default of every optional field. */

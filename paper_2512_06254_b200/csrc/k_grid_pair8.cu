@@ -128,18 +128,17 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                 if (count_rej) ++n_off;
             }
         };
-        // software pipeline: raw inputs and cell (+ density) of batch b + 1 are requested once batch
-        // b's have been used, INTO THE SAME REGISTERS (no current/next copies), and arrive while the
-        // batch is accumulated; the channel scale s_c runs two batches ahead
-        Raw raw;
-        raw.a = raw.b = make_float2(0.0f, 0.0f); raw.wa = raw.wb = 0.0f; raw.fl = 0u; raw.s = 0.0;
-        Cell cell;
-        cell.key = kNoKey; cell.sh = 0u; cell.xu = cell.xv = 0.0f; cell.dens = 1.0f;
+        // software pipeline: raw inputs and cell (+ density) of batch b + 1 are requested while
+        // batch b is processed; the channel scale s_c runs two batches ahead
+        Raw nxt;
+        nxt.a = nxt.b = make_float2(0.0f, 0.0f); nxt.wa = nxt.wb = 0.0f; nxt.fl = 0u; nxt.s = 0.0;
+        Cell cnxt;
+        cnxt.key = kNoKey; cnxt.sh = 0u; cnxt.xu = cnxt.xv = 0.0f; cnxt.dens = 1.0f;
         double s_ahead = 0.0;
         if (c_lo < c_hi) {
-            load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c_lo, c_lo, raw);
+            load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c_lo, c_lo, nxt);
             if (PIPE) {
-                locate(__ldg(g.s + c_lo), cell);
+                locate(__ldg(g.s + c_lo), cnxt);
                 if (c_lo + kBatch < c_hi) s_ahead = __ldg(g.s + c_lo + kBatch);
             }
         }
@@ -148,82 +147,87 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
             // ---------------- pre-process one sample per lane ----------------
             {
                 const int c = c_lo + b;
-                const bool live = c < c_hi;
-                if (!PIPE) {
-                    cell.key = kNoKey;
-                    if (live) locate(raw.s, cell);
-                }
-                // a flagged sample keeps its own cell as key (z = 0): it moves the window exactly as
-                // its unflagged neighbours do and never takes the slow path; the record of a sample
-                // that contributes nothing has z = 0 and finite taps
-                const unsigned key = live ? cell.key : kNoKey;
-                const bool on = key != kNoKey;
-                constexpr unsigned fmask_b = MODE == 2 ? 0x0000ff00u : 0xff000000u;
-                const float wa = (on && weight_ok(raw.wa) && !(raw.fl & 0x000000ffu)) ? raw.wa : 0.0f;
-                const float wb = (on && weight_ok(raw.wb) && !(raw.fl & fmask_b)) ? raw.wb : 0.0f;
-                const float wI = wa + wb;
-                float tk = 1.0f;
-                bool mine = true;
-                if (CHEB && wI > 0.0f) {
-                    // Eq. 19: slab of this sample and its position s_q in it (G24); T_k(s_q) by the
-                    // three-term recurrence in fp64 (T_k amplifies rounding by ~k^2)
-                    const double r3 = __dmul_rn(rho3, raw.s);
-                    int pq = 0;
-                    double sq = 0.0;
-                    if (cheb.d > 0.0) {
-                        pq = min((int)floor((r3 - cheb.r3_min) / (2.0 * cheb.d)), cheb.n_slab - 1);
-                        sq = (r3 - (cheb.r3_min + (2.0 * (double)pq + 1.0) * cheb.d)) / cheb.d;
+                const Raw cur = nxt;
+                Cell cell = cnxt;
+                if (c + kBatch < c_hi && b + kBatch < strip_len) {
+                    load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c + kBatch, c + kBatch, nxt);
+                    if (PIPE) {
+                        locate(s_ahead, cnxt);
+                        if (c + 2 * kBatch < c_hi) s_ahead = __ldg(g.s + c + 2 * kBatch);
                     }
-                    mine = pq == cheb.p;
-                    double t0 = 1.0, t1 = sq;
-                    for (int kk = 1; kk < cheb.k; ++kk) {
-                        const double t2 = fma(2.0 * sq, t1, -t0);
-                        t0 = t1; t1 = t2;
-                    }
-                    tk = (float)(cheb.k == 0 ? 1.0 : t1);
                 }
-                const bool valid = wI > 0.0f && mine;
-                if (on && !(wI > 0.0f) && count_rej) ++n_flag;
-                if (valid && count) ++n_grid;
-                // z = w_a Vis_a + w_b Vis_b; a zero-weight hand is skipped (its data may be NaN)
-                float zx = 0.0f, zy = 0.0f;
-                if (wa > 0.0f) { zx = wa * raw.a.x; zy = wa * raw.a.y; }
-                if (wb > 0.0f) { zx = fmaf(wb, raw.b.x, zx); zy = fmaf(wb, raw.b.y, zy); }
-                if (CHEB) { zx *= tk; zy *= tk; }
-                if (!valid) zx = zy = 0.0f;
+                if (!PIPE && c < c_hi) locate(cur.s, cell);
+                unsigned key = kNoKey;
+                bool valid = false;
+                float wI = 0.0f, zx = 0.0f, zy = 0.0f, pv0 = 0.0f;
+                if (c < c_hi && cell.key != kNoKey) {
+                    // a flagged sample keeps its own cell as key (z = 0, zero taps): it moves the
+                    // window exactly as its unflagged neighbours do and never takes the slow path
+                    key = cell.key;
+                    constexpr unsigned fmask_b = MODE == 2 ? 0x0000ff00u : 0xff000000u;
+                    const float wa = (weight_ok(cur.wa) && !(cur.fl & 0x000000ffu)) ? cur.wa : 0.0f;
+                    const float wb = (weight_ok(cur.wb) && !(cur.fl & fmask_b)) ? cur.wb : 0.0f;
+                    wI = wa + wb;
+                    float tk = 1.0f;
+                    bool mine = true;
+                    if (CHEB && wI > 0.0f) {
+                        // Eq. 19: slab of this sample and its position s_q in it (G24); T_k(s_q) by the
+                        // three-term recurrence in fp64 (T_k amplifies rounding by ~k^2)
+                        const double r3 = __dmul_rn(rho3, cur.s);
+                        int pq = 0;
+                        double sq = 0.0;
+                        if (cheb.d > 0.0) {
+                            pq = min((int)floor((r3 - cheb.r3_min) / (2.0 * cheb.d)), cheb.n_slab - 1);
+                            sq = (r3 - (cheb.r3_min + (2.0 * (double)pq + 1.0) * cheb.d)) / cheb.d;
+                        }
+                        mine = pq == cheb.p;
+                        double t0 = 1.0, t1 = sq;
+                        for (int kk = 1; kk < cheb.k; ++kk) {
+                            const double t2 = fma(2.0 * sq, t1, -t0);
+                            t0 = t1; t1 = t2;
+                        }
+                        tk = (float)(cheb.k == 0 ? 1.0 : t1);
+                    }
+                    if (!(wI > 0.0f)) {
+                        if (count_rej) ++n_flag;
+                    } else if (mine) {
+                        if (count) ++n_grid;
+                        valid = true;
+                        // z = w_a Vis_a + w_b Vis_b; a zero-weight hand is skipped (its data may be NaN)
+                        if (wa > 0.0f) { zx = wa * cur.a.x; zy = wa * cur.a.y; }
+                        if (wb > 0.0f) { zx = fmaf(wb, cur.b.x, zx); zy = fmaf(wb, cur.b.y, zy); }
+                        if (CHEB) { zx *= tk; zy *= tk; }
+                        float pu[kW], pv[kW];
+                        kernel_taps2(cell.xu, cell.xv, pu, pv);
+                        // the 7 taps sit at window offset 0 or 1 on each axis; the free end is zero
+                        const bool su = (cell.sh & 1u) != 0u, sv = (cell.sh & 2u) != 0u;
+                        unsigned wu[kR], wv[kR];
+#pragma unroll
+                        for (int i = 0; i < kR; ++i) {
+                            const float lo_u = i < kW ? pu[i] : 0.0f, hi_u = i > 0 ? pu[i - 1] : 0.0f;
+                            const float lo_v = i < kW ? pv[i] : 0.0f, hi_v = i > 0 ? pv[i - 1] : 0.0f;
+                            wu[i] = __float_as_uint(su ? hi_u : lo_u);
+                            wv[i] = __float_as_uint(sv ? hi_v : lo_v);
+                        }
+                        pv0 = __uint_as_float(wv[0]);
+                        my_rec[1] = make_uint4(wv[1], wv[2], wv[3], wv[4]);
+                        my_rec[2] = make_uint4(wv[5], wv[6], wv[7], 0u);
+                        my_rec[3] = make_uint4(wu[0], wu[1], wu[2], wu[3]);
+                        my_rec[4] = make_uint4(wu[4], wu[5], wu[6], wu[7]);
+                    }
+                }
+                if (!valid) {
+                    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+                    my_rec[1] = zero; my_rec[2] = zero; my_rec[3] = zero; my_rec[4] = zero;
+                }
                 float f = 1.0f;
                 if (has_d) {
                     // the density of a cell whose samples are all flagged is 0: never invert it
                     const float dens = valid ? cell.dens : 1.0f;
                     asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(f) : "f"(dens));
                 }
-                if (!CHEB || count) wpart = fmaf(f, valid ? wI : 0.0f, wpart);
-                const float xu = cell.xu, xv = cell.xv;
-                const bool su = (cell.sh & 1u) != 0u, sv = (cell.sh & 2u) != 0u;
-                // ---- this batch's raw inputs and cell are used up: request the next batch's ----
-                if (c + kBatch < c_hi && b + kBatch < strip_len) {
-                    load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c + kBatch, c + kBatch, raw);
-                    if (PIPE) {
-                        locate(s_ahead, cell);
-                        if (c + 2 * kBatch < c_hi) s_ahead = __ldg(g.s + c + 2 * kBatch);
-                    }
-                }
-                float pu[kW], pv[kW];
-                kernel_taps2(xu, xv, pu, pv);
-                // the 7 taps sit at window offset 0 or 1 on each axis; the free end is zero
-                unsigned wu[kR], wv[kR];
-#pragma unroll
-                for (int i = 0; i < kR; ++i) {
-                    const float lo_u = i < kW ? pu[i] : 0.0f, hi_u = i > 0 ? pu[i - 1] : 0.0f;
-                    const float lo_v = i < kW ? pv[i] : 0.0f, hi_v = i > 0 ? pv[i - 1] : 0.0f;
-                    wu[i] = __float_as_uint(su ? hi_u : lo_u);
-                    wv[i] = __float_as_uint(sv ? hi_v : lo_v);
-                }
-                my_rec[1] = make_uint4(wv[1], wv[2], wv[3], wv[4]);
-                my_rec[2] = make_uint4(wv[5], wv[6], wv[7], 0u);
-                my_rec[3] = make_uint4(wu[0], wu[1], wu[2], wu[3]);
-                my_rec[4] = make_uint4(wu[4], wu[5], wu[6], wu[7]);
-                my_rec[0] = make_uint4(__float_as_uint(zx * f), __float_as_uint(zy * f), key, wv[0]);
+                if (!CHEB || (count && valid)) wpart = fmaf(f, wI, wpart);
+                my_rec[0] = make_uint4(__float_as_uint(zx * f), __float_as_uint(zy * f), key, __float_as_uint(pv0));
             }
             __syncwarp();
             // ---------------- accumulate: every group consumes its 4 records ----------------

@@ -255,6 +255,8 @@ void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const
 inline size_t grid_guard(int G) { return ((size_t)G + 8 + 31) / 32 * 32; }
 void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                             float2 *d_grid, uint8_t *tiles, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
+bool launch_grid_tma(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
+                     float2 *d_grid, uint8_t *tiles, int n_sms, cudaStream_t stream);
 void launch_grid_ws(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                     float2 *d_grid, uint8_t *tiles, int n_sms, cudaStream_t stream);
 void launch_grid_ws_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,

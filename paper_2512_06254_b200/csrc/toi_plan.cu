@@ -289,6 +289,10 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
         launch_grid_pair8(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
     else if (p->cfg.gridder == TOI_GRIDDER_WS)
         launch_grid_ws(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
+    else if (p->cfg.gridder == TOI_GRIDDER_TMA) {
+        if (!launch_grid_tma(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream))
+            launch_grid_pair8(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
+    }
     else
         launch_grid_atomic(g, in, p->d_state, dens, p->d_grid, stream);
     launches += tiles ? 1 : 2;
@@ -388,7 +392,8 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     if (W != kW) return fail(nullptr, TOI_ERR_UNSUPPORTED, "only kernel_support = 7 is built");
     if (cfg->weighting != TOI_WEIGHT_NATURAL && cfg->weighting != TOI_WEIGHT_UNIFORM) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown weighting");
     if (cfg->input_location != TOI_MEM_HOST && cfg->input_location != TOI_MEM_DEVICE) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown input_location");
-    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC && cfg->gridder != TOI_GRIDDER_WS)
+    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC && cfg->gridder != TOI_GRIDDER_WS &&
+        cfg->gridder != TOI_GRIDDER_TMA)
         return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown gridder");
     if ((cfg->enable_3d != 0 && cfg->enable_3d != 1) || (cfg->debug_keep_grid != 0 && cfg->debug_keep_grid != 1))
         return fail(nullptr, TOI_ERR_INVALID_ARG, "enable_3d and debug_keep_grid must be 0 or 1");
