@@ -45,7 +45,7 @@ def parse_args():
     ap.add_argument("--workload", type=int, default=2, choices=[1, 2, 4, 5],
                     help="BASELINE.json config id (2 = configs[1], the metric's workload)")
     ap.add_argument("--weighting", default=None, choices=[None, "natural", "uniform"])
-    ap.add_argument("--gridder", default="sliding", choices=["sliding", "atomic", "ws", "tma"])
+    ap.add_argument("--gridder", default="sliding", choices=["sliding", "atomic"])
     ap.add_argument("--stream-snapshots", type=int, default=1500,
                     help="length of the streamed (configs[2]) run reported under `stream`; 0 = skip")
     ap.add_argument("--stream-pool", type=int, default=16,
@@ -247,7 +247,7 @@ def roofline_of(wl, weighting, stages, stages_min, peak, peak_src, kernel):
     ab = algorithmic_bytes(wl, weighting)
     grid_ms = stages["ms_grid"] + stages["ms_clear"]
     achieved = ab["gridding"] / (grid_ms * 1e-3) / 1e9
-    return {"bound": "hbm", "kernel": kernel + " + k_clear_tiles (sparse clear of the grid, and of the density map)",
+    return {"bound": "hbm", "kernel": kernel + " + k_clear_tiles (sparse clear of the gridding grid; under uniform weighting the same launch also clears the density map)",
             "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
             "frac_of_8tbs_nominal": achieved / 8000.0, "peak_source": peak_src,
             "algorithmic_bytes": ab["gridding"], "ms": grid_ms, "ms_kernel": stages["ms_grid"],
@@ -297,7 +297,7 @@ def run_ours(args):
     toi.load()
     wl, weighting = workload(args)
     wt = toi.TOI_WEIGHT_UNIFORM if weighting == "uniform" else toi.TOI_WEIGHT_NATURAL
-    gridder = {"sliding": toi.TOI_GRIDDER_SLIDING, "atomic": toi.TOI_GRIDDER_ATOMIC, "ws": toi.TOI_GRIDDER_WS, "tma": toi.TOI_GRIDDER_TMA}[args.gridder]
+    gridder = {"sliding": toi.TOI_GRIDDER_SLIDING, "atomic": toi.TOI_GRIDDER_ATOMIC}[args.gridder]
     S = wl.n_baselines * wl.n_chan
     N = wl.image_size
     snap = make_inputs(wl, "cuda")            # seeded generator, on the device; every rank the same shape
@@ -521,7 +521,7 @@ def main():
         return
     ab = algorithmic_bytes(wl, weighting)
     peak, peak_src = measured_peaks()
-    kernel = {"sliding": "k_grid_pair8", "atomic": "k_grid_atomic", "ws": "k_grid_ws", "tma": "k_grid_tma"}[args.gridder]
+    kernel = {"sliding": "k_grid_pair8", "atomic": "k_grid_atomic"}[args.gridder]
     roofline = roofline_of(wl, weighting, r["stages"], r["stages_min"], peak, peak_src, kernel)
     tr = NCU_TRAFFIC.get((str(args.workload), weighting, args.gridder))
     roofline["traffic"] = None if tr is None else tr["bytes"]

@@ -53,7 +53,7 @@ enum { TOI_MEM_HOST = 0, TOI_MEM_DEVICE = 1 };
  * float atomics, k_grid_atomic.cu) is the ncu comparison point the design replaces and a second,
  * structurally different implementation for the parity tests.  Both give the same image within
  * the parity bars. */
-enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1, TOI_GRIDDER_WS = 2, TOI_GRIDDER_TMA = 3 };
+enum { TOI_GRIDDER_SLIDING = 0, TOI_GRIDDER_ATOMIC = 1 };
 
 /* The paper's inputs (Measurement Set, image size, cell size) plus the knobs the
  * paper leaves open.  Zero selects the default of every optional field. */
@@ -88,9 +88,10 @@ typedef struct {
     double wsum;                /* sum_q f_q w_I,q over gridded samples: Eq. 7's N_vis */
     int64_t n_gridded, n_off_grid, n_flagged;
     float ms_h2d, ms_planefit, ms_weight, ms_grid, ms_fft, ms_crop, ms_total;
-    float ms_clear;             /* sparse clear of the gridding grid (+ density map): only the 32x32-cell
-                                   tiles this snapshot touched are zeroed again, after the first FFT
-                                   pass has read the grid; not included in ms_fft */
+    float ms_clear;             /* sparse clear of the gridding grid (and, in the same launch, of the
+                                   density map): only the 128x8-cell tiles this snapshot touched are
+                                   zeroed again, after the first FFT pass has read the grid; not
+                                   included in ms_fft */
 } toi_snapshot_info;
 
 /* Allocate everything: device input slots, gridding grid, FFT workspace, tile maps, image ring,

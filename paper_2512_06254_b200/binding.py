@@ -18,7 +18,7 @@ TOI_ERR_INVALID_ARG, TOI_ERR_CUDA, TOI_ERR_CUFFT, TOI_ERR_NOMEM = -1, -2, -3, -4
 TOI_ERR_DEGENERATE_GEOMETRY, TOI_ERR_CALLBACK, TOI_ERR_UNSUPPORTED = -5, -6, -7
 TOI_WEIGHT_NATURAL, TOI_WEIGHT_UNIFORM = 0, 1
 TOI_MEM_HOST, TOI_MEM_DEVICE = 0, 1
-TOI_GRIDDER_SLIDING, TOI_GRIDDER_ATOMIC, TOI_GRIDDER_WS, TOI_GRIDDER_TMA = 0, 1, 2, 3
+TOI_GRIDDER_SLIDING, TOI_GRIDDER_ATOMIC = 0, 1
 TOI_REPROJECT_EXACT, TOI_REPROJECT_PAPER = 0, 1
 TOI_OUT_TILTED, TOI_OUT_REPROJECT_EXACT, TOI_OUT_REPROJECT_PAPER = 0, 1, 2
 

@@ -2,7 +2,7 @@
 //
 // A snapshot touches 2-3 % of the G x G cells (3091 of 16384 32x32 tiles at
 // config 2), so zero-filling the whole grid for every snapshot (134 MB of HBM writes at config 2,
-// 2.1 GB at config 4) is wasted traffic.  The gridder and the density pass mark the 32 x 32-cell
+// 2.1 GB at config 4) is wasted traffic.  The gridder and the density pass mark the 128 x 8-cell
 // tiles they may write in a byte map; once the first FFT pass has read the grid (out of place, into
 // the FFT workspace) this kernel zeroes exactly those tiles again and resets the map, so the next
 // snapshot finds a zero grid.  The grid is zero-filled in full once, at plan creation.
@@ -13,57 +13,65 @@ namespace {
 
 // One warp takes kTilesPerWarp consecutive map entries and clears the marked tiles one after the
 // other (few tiles per warp: the marked tiles cluster around the uv origin, and a warp that finds
-// all of its entries marked must not become the tail of the kernel): a tile row is kTile elements
-// = 32 x 8 B (complex64) or 16 x 8 B (float32) -- 8-byte stores keep every even G legal (a row
-// pitch of G * 4 B is then only 8-byte aligned).
+// all of its entries marked must not become the tail of the kernel).  A tile row of the grid is
+// kTileW complex64 = 1 KB, written with 8-byte stores.
+//
+// The density map (uniform weighting) needs no map of its own: the density pass writes the centre
+// cells of the samples -- inside the tiles the gridder marks for the same samples' windows -- and
+// their mirror cells (-iu, -iv), i.e. array index (G - x, G - y) for (x, y).  For every marked tile
+// the same rectangle of the density map and its point mirror are zeroed (4-byte stores: the mirrored
+// rectangle starts on any column).
 constexpr int kTilesPerWarp = 4;
 
-template <typename T>
 __global__ void __launch_bounds__(256)
-k_clear_tiles(T *__restrict__ buf, int G, uint8_t *__restrict__ map, int tpr)
+k_clear_tiles(float2 *__restrict__ grid, float *__restrict__ dens, int G, uint8_t *__restrict__ map, int tpr,
+              long long n_tiles)
 {
     const int lane = threadIdx.x & 31;
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const long long t0 = warp * kTilesPerWarp;
-    const long long n_tiles = (long long)tpr * tpr;
     if (t0 >= n_tiles) return;
     const long long mine = t0 + lane;
     const bool dirty = lane < kTilesPerWarp && mine < n_tiles && map[mine] != 0;
     if (dirty) map[mine] = 0;
     unsigned todo = __ballot_sync(0xffffffffu, dirty);
-    constexpr int kPerStore = 8 / (int)sizeof(T);                 // elements per 8-byte store: 1 or 2
-    constexpr int kLanesPerRow = kTile / kPerStore;               // 32 or 16
-    constexpr int kRowsPerPass = 32 / kLanesPerRow;               // 1 or 2
     while (todo) {
         const int b = __ffs(todo) - 1;
         todo &= todo - 1;
         const long long t = t0 + b;
-        const int ty = (int)(t / tpr), tx = (int)(t % tpr);
-        const int col = tx * kTile + (lane % kLanesPerRow) * kPerStore;
-        if (col >= G) continue;                                   // G even: an 8-byte store never straddles the edge
-        const int r0 = lane / kLanesPerRow;
-        const int rows = min(kTile, G - ty * kTile);
-        uint2 *p = reinterpret_cast<uint2 *>(buf + (size_t)(ty * kTile + r0) * G + col);
-        const size_t pitch = (size_t)kRowsPerPass * G * sizeof(T) / sizeof(uint2);
-#pragma unroll 8
-        for (int r = r0; r < rows; r += kRowsPerPass, p += pitch) *p = make_uint2(0u, 0u);
+        const int x0 = (int)(t % tpr) * kTileW, y0 = (int)(t / tpr) * kTileH;
+        const int rows = min(kTileH, G - y0);
+        float2 *row = grid + (size_t)y0 * G + x0;
+        for (int r = 0; r < rows; ++r, row += G) {
+#pragma unroll
+            for (int k = 0; k < kTileW / 32; ++k)
+                if (x0 + k * 32 + lane < G) row[k * 32 + lane] = make_float2(0.0f, 0.0f);
+        }
+        if (dens != nullptr) {
+            for (int r = 0; r < rows; ++r) {
+                float *own = dens + (size_t)(y0 + r) * G;
+                const int ym = G - (y0 + r);                      // mirrored row; G itself is outside
+                float *mir = dens + (size_t)(ym < G ? ym : 0) * G;
+#pragma unroll
+                for (int k = 0; k < kTileW / 32; ++k) {
+                    const int x = x0 + k * 32 + lane, xm = G - x;
+                    if (x < G) own[x] = 0.0f;
+                    if (x < G && ym < G && xm < G) mir[xm] = 0.0f;
+                }
+            }
+        }
     }
 }
 
 }  // namespace
 
-void launch_clear_tiles(float2 *d_grid, int G, uint8_t *d_map, cudaStream_t stream)
+// grid (and density map if not null): zero the tiles marked in d_map, reset the map
+void launch_clear_tiles(float2 *d_grid, float *d_density, int G, uint8_t *d_map, cudaStream_t stream)
 {
     const int tpr = tiles_per_row(G);
-    const long long warps = ((long long)tpr * tpr + kTilesPerWarp - 1) / kTilesPerWarp;
-    k_clear_tiles<float2><<<(unsigned)((warps + 7) / 8), 256, 0, stream>>>(d_grid, G, d_map, tpr);
-}
-
-void launch_clear_tiles(float *d_density, int G, uint8_t *d_map, cudaStream_t stream)
-{
-    const int tpr = tiles_per_row(G);
-    const long long warps = ((long long)tpr * tpr + kTilesPerWarp - 1) / kTilesPerWarp;
-    k_clear_tiles<float><<<(unsigned)((warps + 7) / 8), 256, 0, stream>>>(d_density, G, d_map, tpr);
+    const long long n_tiles = (long long)tpr * tile_rows(G);
+    const long long warps = (n_tiles + kTilesPerWarp - 1) / kTilesPerWarp;
+    k_clear_tiles<<<(unsigned)((warps + 7) / 8), 256, 0, stream>>>(d_grid, d_density, G, d_map, tpr, n_tiles);
 }
 
 }  // namespace toi

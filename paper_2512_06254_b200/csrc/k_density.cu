@@ -15,8 +15,7 @@ constexpr int kChunks = 4;   // 32-channel chunks per warp: all their loads are 
 // one LDG.32 per sample; otherwise the generic per-hand loads of sample_weights().
 template <bool FAST>
 __global__ void __launch_bounds__(256)
-k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__restrict__ D,
-          uint8_t *__restrict__ tiles)
+k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__restrict__ D)
 {
     if (st->status != TOI_OK) return;
     const int lane = threadIdx.x & 31;
@@ -46,7 +45,6 @@ k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__rest
     rotate_baseline(st->V, in.uvw + 3 * j, rho1, rho2);
     const int G = g.G;
     float *const Dc = D + centre_index(0, 0, G);
-    const int tpr = tiles_per_row(G), h = G >> 1;
 
 #pragma unroll
     for (int u = 0; u < kChunks; ++u) {
@@ -87,30 +85,22 @@ k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__rest
             const long long o = (long long)iv * G + iu;
             atomicAdd(Dc + o, sum);
             atomicAdd(Dc - o, sum);                       // the mirror cell (-iu, -iv)
-            // sparse clear (k_clear.cu): the tiles of the two cells just written
-            // (checked first: an L1 hit instead of a store that thousands of runs would send to the
-            // same few L2 sectors; a stale 0 only repeats the store)
-            uint8_t *const ta = tiles + ((iv + h) / kTile) * tpr + (iu + h) / kTile;
-            uint8_t *const tb = tiles + ((h - iv) / kTile) * tpr + (h - iu) / kTile;
-            if (*ta == 0) *ta = 1;
-            if (*tb == 0) *tb = 1;
         }
     }
 }
 
 }  // namespace
 
-void launch_density(const Geometry &g, const Inputs &in, SnapState *st, float *d_density, uint8_t *tiles,
-                    cudaStream_t stream)
+void launch_density(const Geometry &g, const Inputs &in, SnapState *st, float *d_density, cudaStream_t stream)
 {
     const long long warps = (long long)g.n_b * ((g.n_c + 32 * kChunks - 1) / (32 * kChunks));
     const int threads = 256;
     const long long blocks = (warps * 32 + threads - 1) / threads;
     const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags;
     if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
-        k_density<true><<<(unsigned)blocks, threads, 0, stream>>>(g, in, st, d_density, tiles);
+        k_density<true><<<(unsigned)blocks, threads, 0, stream>>>(g, in, st, d_density);
     else
-        k_density<false><<<(unsigned)blocks, threads, 0, stream>>>(g, in, st, d_density, tiles);
+        k_density<false><<<(unsigned)blocks, threads, 0, stream>>>(g, in, st, d_density);
 }
 
 }  // namespace toi

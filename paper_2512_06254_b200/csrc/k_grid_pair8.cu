@@ -25,6 +25,16 @@
 namespace toi {
 namespace {
 
+// The task queue: rows [0, j1) are cut into tasks of 8 strips of strip1 channels, the remaining rows
+// into tasks of 8 strips of strip2 (about half as long).  Tasks are claimed in ascending order, so
+// the kernel's last ~fifth of work comes in small pieces: warps then finish within half a small
+// task of one another instead of half a large one (the tail was 7 % of the warp-time, ncu
+// sm__warps_active 14.9 of 16), at the price of one more window flush per strip there.
+struct TaskShape {
+    int strip1, tpr1, strip2, tpr2;
+    unsigned t1, j1, n_tasks;       // tasks of the first kind, rows they cover, all tasks
+};
+
 constexpr int kWarps = 8;         // warps per CTA
 constexpr int ctas_per_sm(bool) { return 2; }          // 16 warps/SM at <= 128 registers (4 x 4 warps measured 1 % slower)
 
@@ -35,8 +45,7 @@ constexpr int ctas_per_sm(bool) { return 2; }          // 16 warps/SM at <= 128 
 template <int MODE, int OPT, bool PIPE, bool CHEB>
 __global__ void __launch_bounds__(kWarps * 32, ctas_per_sm(PIPE))
 k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__restrict__ D,
-            float2 *__restrict__ grid, uint8_t *__restrict__ tiles, int strip_len, int tasks_per_row,
-            unsigned n_tasks, ChebArgs cheb)
+            float2 *__restrict__ grid, uint8_t *__restrict__ tiles, TaskShape shape, ChebArgs cheb)
 {
     static_assert(!(PIPE && CHEB), "the Chebyshev pass computes the cell in place");
     __shared__ uint4 s_rec[kWarps * kWarpQuads];
@@ -69,10 +78,13 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
     if (lane == 0) task_ahead = atomicAdd(&st->task_counter, 1u);
     for (;;) {
         const unsigned task = __shfl_sync(0xffffffffu, task_ahead, 0);
-        if (task >= n_tasks) break;
+        if (task >= shape.n_tasks) break;
         if (lane == 0) task_ahead = atomicAdd(&st->task_counter, 1u);
-        const int j = (int)(task / (unsigned)tasks_per_row);
-        const int c_task = (int)(task % (unsigned)tasks_per_row) * (kGroups * strip_len);
+        const bool big = task < shape.t1;
+        const unsigned t_in = big ? task : task - shape.t1, tpr = (unsigned)(big ? shape.tpr1 : shape.tpr2);
+        const int strip_len = big ? shape.strip1 : shape.strip2;
+        const int j = (int)((big ? 0u : shape.j1) + t_in / tpr);
+        const int c_task = (int)(t_in % tpr) * (kGroups * strip_len);
         double rho1, rho2;
         rotate_baseline(st->V, in.uvw + 3 * j, rho1, rho2);
         const double rho3 = CHEB ? rotate_row3(st->V, in.uvw + 3 * j) : 0.0;
@@ -95,8 +107,8 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
             const int ju = __shfl_xor_sync(0xffffffffu, iu, 1), jv = __shfl_xor_sync(0xffffffffu, iv, 1);
             if (some && L == 0) {
                 const int h = G >> 1, tpr = tiles_per_row(G);
-                const int x0 = max(min(iu, ju) - 4 + h, 0) / kTile, x1 = min(max(iu, ju) + 4 + h, G - 1) / kTile;
-                const int y0 = max(min(iv, jv) - 4 + h, 0) / kTile, y1 = min(max(iv, jv) + 4 + h, G - 1) / kTile;
+                const int x0 = max(min(iu, ju) - 4 + h, 0) / kTileW, x1 = min(max(iu, ju) + 4 + h, G - 1) / kTileW;
+                const int y0 = max(min(iv, jv) - 4 + h, 0) / kTileH, y1 = min(max(iv, jv) + 4 + h, G - 1) / kTileH;
                 for (int ty = y0; ty <= y1; ++ty)
                     for (int tx = x0; tx <= x1; ++tx)
                         if (tiles[ty * tpr + tx] == 0) tiles[ty * tpr + tx] = 1;   // L1 hit instead of a store, mostly
@@ -256,10 +268,9 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
 
 template <int MODE>
 void launch_mode(int opt, dim3 grid, dim3 block, cudaStream_t stream, const Geometry &g, const Inputs &in,
-                 SnapState *st, const float *D, float2 *d_grid, uint8_t *tiles, int strip, int tasks_per_row,
-                 unsigned n_tasks)
+                 SnapState *st, const float *D, float2 *d_grid, uint8_t *tiles, const TaskShape &shape)
 {
-#define TOI_LAUNCH(O, P) k_grid_pair8<MODE, O, P, false><<<grid, block, 0, stream>>>(g, in, st, D, d_grid, tiles, strip, tasks_per_row, n_tasks, ChebArgs())
+#define TOI_LAUNCH(O, P) k_grid_pair8<MODE, O, P, false><<<grid, block, 0, stream>>>(g, in, st, D, d_grid, tiles, shape, ChebArgs())
     switch (opt) {
     case kHasW | kHasF | kHasD: TOI_LAUNCH(kHasW | kHasF | kHasD, true); break;
     case kHasW | kHasF: TOI_LAUNCH(kHasW | kHasF, false); break;
@@ -274,46 +285,57 @@ void launch_mode(int opt, dim3 grid, dim3 block, cudaStream_t stream, const Geom
 
 }  // namespace
 
+namespace {
+
+// strip length (channels per group per task): 8 strips per task; aim at >= 6 tasks per resident
+// warp, within [16, 128] channels and a multiple of the 4-sample batch; the last fifth of the rows
+// gets strips of about half that length (struct TaskShape)
+TaskShape task_shape(const Geometry &g, int n_sms, int ctas_per_sm_, long long *ctas)
+{
+    TaskShape sh;
+    const long long warps = (long long)ctas_per_sm_ * n_sms * kWarps;
+    const long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
+    sh.strip1 = pick_strip(g.n_c, kGroups, kBatch, want, 16, 128);
+    sh.tpr1 = (g.n_c + kGroups * sh.strip1 - 1) / (kGroups * sh.strip1);
+    sh.strip2 = pick_strip(g.n_c, kGroups, kBatch, sh.strip1 / 2, 16, 128);
+    sh.tpr2 = (g.n_c + kGroups * sh.strip2 - 1) / (kGroups * sh.strip2);
+    sh.j1 = sh.strip2 < sh.strip1 ? (unsigned)(g.n_b - g.n_b / 5) : (unsigned)g.n_b;
+    sh.t1 = sh.j1 * (unsigned)sh.tpr1;
+    const long long n_tasks = (long long)sh.t1 + (long long)(g.n_b - (int)sh.j1) * sh.tpr2;
+    sh.n_tasks = (unsigned)n_tasks;
+    *ctas = (n_tasks + kWarps - 1) / kWarps;
+    if (*ctas > (long long)ctas_per_sm_ * n_sms) *ctas = (long long)ctas_per_sm_ * n_sms;   // persistent CTAs pull from the queue
+    return sh;
+}
+
+}  // namespace
+
 // G <= 32768 (toi_plan_create checks): a window base must fit the packed 16-bit key.
 void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                        float2 *d_grid, uint8_t *tiles, int n_sms, cudaStream_t stream)
 {
-    // strip length (channels per group per task): 8 strips per task; aim at >= 6 tasks per resident
-    // warp, within [16, 128] channels and a multiple of the 4-sample batch
-    const int kCtasPerSm = ctas_per_sm(d_density != nullptr);
-    const long long warps = (long long)kCtasPerSm * n_sms * kWarps;
-    const long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
-    const int strip = pick_strip(g.n_c, kGroups, kBatch, want, 16, 128);
-    const int tasks_per_row = (g.n_c + kGroups * strip - 1) / (kGroups * strip);
-    const long long n_tasks = (long long)g.n_b * tasks_per_row;
-    long long ctas = (n_tasks + kWarps - 1) / kWarps;
-    if (ctas > (long long)kCtasPerSm * n_sms) ctas = (long long)kCtasPerSm * n_sms;   // persistent CTAs pull from the queue
+    long long ctas = 0;
+    const TaskShape shape = task_shape(g, n_sms, ctas_per_sm(d_density != nullptr), &ctas);
     const dim3 grid((unsigned)ctas), block(kWarps * 32);
     const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags, av = (uintptr_t)in.vis;
     const int opt = (in.weights ? kHasW : 0) | (in.flags ? kHasF : 0) | (d_density ? kHasD : 0);
     if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
-        launch_mode<4>(opt, grid, block, stream, g, in, st, d_density, d_grid, tiles, strip, tasks_per_row, (unsigned)n_tasks);
+        launch_mode<4>(opt, grid, block, stream, g, in, st, d_density, d_grid, tiles, shape);
     else if (g.n_p == 2 && g.pol_a == 0 && g.pol_b == 1 && (av & 15) == 0 && (aw & 7) == 0 && (af & 1) == 0)
-        launch_mode<2>(opt, grid, block, stream, g, in, st, d_density, d_grid, tiles, strip, tasks_per_row, (unsigned)n_tasks);
+        launch_mode<2>(opt, grid, block, stream, g, in, st, d_density, d_grid, tiles, shape);
     else
-        launch_mode<0>(-1, grid, block, stream, g, in, st, d_density, d_grid, tiles, strip, tasks_per_row, (unsigned)n_tasks);
+        launch_mode<0>(-1, grid, block, stream, g, in, st, d_density, d_grid, tiles, shape);
 }
 
 // One Chebyshev-moment pass of the near-coplanar mode.
 void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                             float2 *d_grid, uint8_t *tiles, int n_sms, const ChebArgs &cheb, cudaStream_t stream)
 {
-    const int kCtasPerSm = ctas_per_sm(false);
-    const long long warps = (long long)kCtasPerSm * n_sms * kWarps;
-    const long long want = ((long long)g.n_b * g.n_c) / (kGroups * 6 * warps);
-    const int strip = pick_strip(g.n_c, kGroups, kBatch, want, 16, 128);
-    const int tasks_per_row = (g.n_c + kGroups * strip - 1) / (kGroups * strip);
-    const long long n_tasks = (long long)g.n_b * tasks_per_row;
-    long long ctas = (n_tasks + kWarps - 1) / kWarps;
-    if (ctas > (long long)kCtasPerSm * n_sms) ctas = (long long)kCtasPerSm * n_sms;
+    long long ctas = 0;
+    const TaskShape shape = task_shape(g, n_sms, ctas_per_sm(false), &ctas);
     const dim3 grid((unsigned)ctas), block(kWarps * 32);
     const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags, av = (uintptr_t)in.vis;
-#define TOI_LAUNCH_CHEB(M) k_grid_pair8<M, -1, false, true><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, tiles, strip, tasks_per_row, (unsigned)n_tasks, cheb)
+#define TOI_LAUNCH_CHEB(M) k_grid_pair8<M, -1, false, true><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, tiles, shape, cheb)
     if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
         TOI_LAUNCH_CHEB(4);
     else if (g.n_p == 2 && g.pol_a == 0 && g.pol_b == 1 && (av & 15) == 0 && (aw & 7) == 0 && (af & 1) == 0)

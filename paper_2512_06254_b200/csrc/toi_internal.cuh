@@ -14,8 +14,11 @@ constexpr int kW = 7;           // kernel support (G9)
 constexpr int kH = 3;           // (W-1)/2
 constexpr float kBetaK = 16.1f; // 2.30 * W
 constexpr int kOffGrid = INT32_MIN;
-constexpr int kTile = 32;       // side of the tiles of the sparse-clear maps, cells (k_clear.cu)
-inline __host__ __device__ int tiles_per_row(int G) { return (G + kTile - 1) / kTile; }
+// tiles of the sparse-clear maps (k_clear.cu): 128 cells wide (1 KB of complex64 per row: whole DRAM
+// bursts) and 8 rows high
+constexpr int kTileW = 128, kTileH = 8;
+inline __host__ __device__ int tiles_per_row(int G) { return (G + kTileW - 1) / kTileW; }
+inline __host__ __device__ int tile_rows(int G) { return (G + kTileH - 1) / kTileH; }
 
 // Device-resident per-snapshot state: written by k_planefit, accumulated by the weighting and
 // gridding kernels, read by k_correct_crop.  No host round trip between the stages.
@@ -241,10 +244,10 @@ inline int pick_strip(int n_c, int groups, int batch, long long want, int lo, in
 // ---- host-side launchers, one per translation unit -------------------------------------------
 void launch_planefit(const Geometry &g, const double *d_uvw, double S1, double S2, const double *d_V_inject,
                      SnapState *st, cudaStream_t stream);
-// `tiles`: byte map of the kTile x kTile-cell tiles of the grid (resp. density map) the kernel may
-// write -- it sets the entries, launch_clear_tiles zeroes those tiles again and resets them.
-void launch_density(const Geometry &g, const Inputs &in, SnapState *st, float *d_density, uint8_t *tiles,
-                    cudaStream_t stream);
+// `tiles`: byte map of the kTileW x kTileH-cell tiles of the grid the gridder may write -- it sets the
+// entries, launch_clear_tiles zeroes those tiles (and the density map under and opposite them) again
+// and resets the entries.
+void launch_density(const Geometry &g, const Inputs &in, SnapState *st, float *d_density, cudaStream_t stream);
 void launch_grid_atomic(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                         float2 *d_grid, cudaStream_t stream);
 // tiles == nullptr: the caller has marked every tile itself (channel scales not monotone)
@@ -255,14 +258,7 @@ void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const
 inline size_t grid_guard(int G) { return ((size_t)G + 8 + 31) / 32 * 32; }
 void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                             float2 *d_grid, uint8_t *tiles, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
-bool launch_grid_tma(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                     float2 *d_grid, uint8_t *tiles, int n_sms, cudaStream_t stream);
-void launch_grid_ws(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                    float2 *d_grid, uint8_t *tiles, int n_sms, cudaStream_t stream);
-void launch_grid_ws_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
-                         float2 *d_grid, uint8_t *tiles, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
-void launch_clear_tiles(float2 *d_grid, int G, uint8_t *d_map, cudaStream_t stream);
-void launch_clear_tiles(float *d_density, int G, uint8_t *d_map, cudaStream_t stream);
+void launch_clear_tiles(float2 *d_grid, float *d_density, int G, uint8_t *d_map, cudaStream_t stream);
 void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s_min, double s_max, double *d_out,
                      cudaStream_t stream);
 size_t bessel_table_doubles(int K);

@@ -42,13 +42,13 @@ struct toi_plan {
     DevSlot dev_in[2];
     toi_snapshot_buffers pin[2] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
     // ONE gridding grid (with guard band) and ONE density map, both zero between snapshots: the
-    // gridder / density pass mark the 32x32-cell tiles they write in a byte map and, once the first
+    // gridder / density pass mark the 128x8-cell tiles they write in a byte map and, once the first
     // FFT pass has read the grid OUT OF PLACE into d_work, only those tiles are zeroed again
     // (k_clear.cu).  The rest of the transform and the crop run on d_work.
     float2 *d_grid = nullptr, *d_grid_alloc = nullptr;   // d_grid = d_grid_alloc + grid_guard(G)
     float2 *d_work = nullptr;                            // FFT workspace, G x G
     float *d_dens = nullptr;
-    uint8_t *d_tiles_grid = nullptr, *d_tiles_dens = nullptr;
+    uint8_t *d_tiles_grid = nullptr;
     size_t n_tiles = 0;
     bool s_monotone = true;      // channel scales monotone: the gridder can bound a strip's tiles by its ends
     float2 *d_grid_keep = nullptr;                       // cfg.debug_keep_grid
@@ -178,7 +178,7 @@ int free_plan(toi_plan *p)
     for (int k = 0; k < EV_COUNT; ++k)
         if (p->ev[k]) cudaEventDestroy(p->ev[k]);
     cudaFree(p->d_grid_alloc); cudaFree(p->d_work); cudaFree(p->d_dens);
-    cudaFree(p->d_tiles_grid); cudaFree(p->d_tiles_dens);
+    cudaFree(p->d_tiles_grid);
     cudaFree(p->d_grid_keep); cudaFree(p->d_dens_keep);
     if (p->ev_done) cudaEventDestroy(p->ev_done);
     if (p->ev_clear0) cudaEventDestroy(p->ev_clear0);
@@ -242,12 +242,8 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, bool clear_density, bo
     }
     ++*launches;
     if (time_clear) CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
-    launch_clear_tiles(p->d_grid, g.G, p->d_tiles_grid, stream);
+    launch_clear_tiles(p->d_grid, clear_density ? p->d_dens : nullptr, g.G, p->d_tiles_grid, stream);
     ++*launches;
-    if (clear_density) {
-        launch_clear_tiles(p->d_dens, g.G, p->d_tiles_dens, stream);
-        ++*launches;
-    }
     if (time_clear) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
     if (p->fft_pruned) {
         cufftComplex *Fhi = F + (g.G - g.N / 2);
@@ -277,7 +273,7 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     // a4: uniform-weighting density pass
     const float *dens = nullptr;
     if (uniform) {
-        launch_density(g, in, p->d_state, p->d_dens, p->d_tiles_dens, stream);
+        launch_density(g, in, p->d_state, p->d_dens, stream);
         dens = p->d_dens;
         ++launches;
     }
@@ -285,14 +281,8 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     // a3 + a5: cell indices and gridding onto the zero grid
     const bool sliding = p->cfg.gridder != TOI_GRIDDER_ATOMIC;
     uint8_t *tiles = gridder_tile_map(p, stream, sliding);
-    if (p->cfg.gridder == TOI_GRIDDER_SLIDING)
+    if (sliding)
         launch_grid_pair8(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
-    else if (p->cfg.gridder == TOI_GRIDDER_WS)
-        launch_grid_ws(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
-    else if (p->cfg.gridder == TOI_GRIDDER_TMA) {
-        if (!launch_grid_tma(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream))
-            launch_grid_pair8(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
-    }
     else
         launch_grid_atomic(g, in, p->d_state, dens, p->d_grid, stream);
     launches += tiles ? 1 : 2;
@@ -392,8 +382,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     if (W != kW) return fail(nullptr, TOI_ERR_UNSUPPORTED, "only kernel_support = 7 is built");
     if (cfg->weighting != TOI_WEIGHT_NATURAL && cfg->weighting != TOI_WEIGHT_UNIFORM) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown weighting");
     if (cfg->input_location != TOI_MEM_HOST && cfg->input_location != TOI_MEM_DEVICE) return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown input_location");
-    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC && cfg->gridder != TOI_GRIDDER_WS &&
-        cfg->gridder != TOI_GRIDDER_TMA)
+    if (cfg->gridder != TOI_GRIDDER_SLIDING && cfg->gridder != TOI_GRIDDER_ATOMIC)
         return fail(nullptr, TOI_ERR_INVALID_ARG, "unknown gridder");
     if ((cfg->enable_3d != 0 && cfg->enable_3d != 1) || (cfg->debug_keep_grid != 0 && cfg->debug_keep_grid != 1))
         return fail(nullptr, TOI_ERR_INVALID_ARG, "enable_3d and debug_keep_grid must be 0 or 1");
@@ -493,14 +482,12 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     CREATE_TRY(cudaMemset(p->d_grid_alloc, 0, (GG + 2 * grid_guard(G)) * sizeof(float2)));
     p->d_grid = p->d_grid_alloc + grid_guard(G);
     CREATE_TRY(cudaMalloc(&p->d_work, GG * sizeof(float2)));
-    p->n_tiles = (size_t)tiles_per_row(G) * tiles_per_row(G);
+    p->n_tiles = (size_t)tiles_per_row(G) * tile_rows(G);
     CREATE_TRY(cudaMalloc(&p->d_tiles_grid, p->n_tiles));
     CREATE_TRY(cudaMemset(p->d_tiles_grid, 0, p->n_tiles));
     if (cfg->weighting == TOI_WEIGHT_UNIFORM) {
         CREATE_TRY(cudaMalloc(&p->d_dens, GG * sizeof(float)));
         CREATE_TRY(cudaMemset(p->d_dens, 0, GG * sizeof(float)));
-        CREATE_TRY(cudaMalloc(&p->d_tiles_dens, p->n_tiles));
-        CREATE_TRY(cudaMemset(p->d_tiles_dens, 0, p->n_tiles));
     }
     CREATE_TRY(cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming));
     CREATE_TRY(cudaEventRecord(p->ev_done, p->s_compute));
@@ -723,7 +710,7 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     const bool uniform = p->cfg.weighting == TOI_WEIGHT_UNIFORM;
     const float *dens = nullptr;
     if (uniform) {
-        launch_density(g, in, p->d_state, p->d_dens, p->d_tiles_dens, stream);
+        launch_density(g, in, p->d_state, p->d_dens, stream);
         dens = p->d_dens;
         ++launches;
     }
@@ -740,10 +727,7 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
             const bool last = sp == slabs_run - 1 && k == K - 1;
             CU_TRY(p, cudaMemsetAsync(&p->d_state->task_counter, 0, sizeof(unsigned int), stream));
             uint8_t *tiles = gridder_tile_map(p, stream, true);
-            if (p->cfg.gridder == TOI_GRIDDER_WS)
-                launch_grid_ws_cheb(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, ca, stream);
-            else
-                launch_grid_pair8_cheb(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, ca, stream);
+            launch_grid_pair8_cheb(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, ca, stream);
             launches += tiles ? 2 : 3;
             if (first && p->keep_grid) {
                 CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));

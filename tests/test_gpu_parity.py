@@ -92,7 +92,7 @@ def _check_all(snap, wl_N, cell, weighting, gridder, pol_a=None, pol_b=None, loc
 # ------------------------------------------------------------------------------------------------
 # config 1 (BASELINE.json configs[0]): the tiny snapshot, natural weighting, both gridders
 # ------------------------------------------------------------------------------------------------
-ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_WS, toi.TOI_GRIDDER_TMA, toi.TOI_GRIDDER_ATOMIC]
+ALL_GRIDDERS = [toi.TOI_GRIDDER_SLIDING, toi.TOI_GRIDDER_ATOMIC]
 
 
 @pytest.mark.parametrize("gridder", ALL_GRIDDERS)
