@@ -84,6 +84,8 @@ class Workload:
     cell_arcsec: float = 1.5
     weighting: str = "uniform"
     pulsar_mjy: float = 0.0       # config 3: on/off pulsar flux (on in 30 % of snapshots)
+    pulsar_ramp_mjy: tuple = ()   # config 4: (first, last) flux of a pulsar ramping linearly over the run
+    n_transients: int = 0         # config 5: faint transients (2-10 mJy), each on in one seeded window of 8-64 snapshots
     n_snapshots: int = 1
 
     @property
@@ -110,9 +112,9 @@ CONFIG1 = Workload("tiny", 1, n_ant=16, n_core=16, flat_array=True, lat_deg=-30.
 CONFIG2 = Workload("meerkat_snapshot", 2)
 CONFIG3 = Workload("meerkat_stream", 3, pulsar_mjy=5.0, n_snapshots=1500)
 CONFIG4 = Workload("wide_deep", 4, n_chan=32768, n_src=400, flag_frac=0.08, image_size=8192,
-                   weighting="natural", n_snapshots=64)
+                   weighting="natural", pulsar_ramp_mjy=(1.0, 20.0), n_snapshots=64)
 CONFIG5 = Workload("low_elevation", 5, n_chan=1024, n_src=10, flux_lo=1.0, flux_hi=5.0,
-                   ha0_deg=-83.3, image_size=4096, weighting="natural", n_snapshots=512)
+                   ha0_deg=-83.3, image_size=4096, weighting="natural", n_transients=12, n_snapshots=512)
 CONFIGS = {1: CONFIG1, 2: CONFIG2, 3: CONFIG3, 4: CONFIG4, 5: CONFIG5}
 
 
@@ -182,6 +184,26 @@ def sky_model(wl: Workload, snapshot: int = 0):
         l = torch.cat([l, torch.tensor([pr * math.cos(pa)], dtype=torch.float64)])
         m = torch.cat([m, torch.tensor([pr * math.sin(pa)], dtype=torch.float64)])
         flux = torch.cat([flux, torch.tensor([wl.pulsar_mjy * 1e-3 if on else 0.0], dtype=torch.float64)])
+    if wl.pulsar_ramp_mjy:
+        one = torch.zeros(1, dtype=torch.int64)
+        lo, hi = wl.pulsar_ramp_mjy
+        f = lo + (hi - lo) * min(max(snapshot, 0), wl.n_snapshots - 1) / max(1, wl.n_snapshots - 1)
+        pr = 0.3 * wl.image_size * beta * math.sqrt(float(hash_uniform(wl.seed, 21, one)))
+        pa = 2.0 * math.pi * float(hash_uniform(wl.seed, 22, one))
+        l = torch.cat([l, torch.tensor([pr * math.cos(pa)], dtype=torch.float64)])
+        m = torch.cat([m, torch.tensor([pr * math.sin(pa)], dtype=torch.float64)])
+        flux = torch.cat([flux, torch.tensor([f * 1e-3], dtype=torch.float64)])
+    if wl.n_transients > 0:
+        t = torch.arange(wl.n_transients, dtype=torch.int64)
+        tr = 0.4 * wl.image_size * beta * torch.sqrt(hash_uniform(wl.seed, 23, t))
+        ta = 2.0 * math.pi * hash_uniform(wl.seed, 24, t)
+        tf = (2.0 + 8.0 * hash_uniform(wl.seed, 25, t)) * 1e-3
+        width = 8 + torch.floor(57.0 * hash_uniform(wl.seed, 26, t)).to(torch.int64)            # 8 .. 64 snapshots
+        start = torch.floor(hash_uniform(wl.seed, 27, t) * (wl.n_snapshots - width).clamp(min=1).to(torch.float64)).to(torch.int64)
+        on = (snapshot >= start) & (snapshot < start + width)
+        l = torch.cat([l, tr * torch.cos(ta)])
+        m = torch.cat([m, tr * torch.sin(ta)])
+        flux = torch.cat([flux, torch.where(on, tf, torch.zeros_like(tf))])
     return l, m, flux
 
 

@@ -95,3 +95,22 @@ def test_oracle_and_cuda_path_share_no_code():
             text = open(os.path.join(ROOT, "oracle", f), errors="replace").read()
             assert not re.search(r"^\s*(from|import)\s+paper_2512_06254_b200", text, flags=re.M), f
             assert '#include "toi' not in text and "csrc/" not in text.replace("paper_2512_06254_b200/csrc", ""), f
+
+
+@pytest.mark.parametrize("G", [16, 18, 136, 198, 202, 384, 4096, 4098, 32766, 32768])
+def test_gridder_window_overhang_stays_inside_the_guard_band(G):
+    """The product gridder flushes an 8 x 8-cell register window whose corner sits on even cells,
+    base = (centre - 3) & ~1, so it can overhang the grid by one row / column (of zeros).  The plan
+    allocates grid_guard(G) = ceil((G + 8) / 32) * 32 cells in front of and behind the grid for that.
+    compute-sanitizer is closed on this GPU pool, so the bound is checked here by enumeration: over all
+    on-grid centre cells (-G/2 + 3 <= i <= G/2 - 4 on both axes) the lowest and highest flat cell index a
+    window can touch must stay within [-guard, G*G + guard)."""
+    h = G // 2
+    guard = (G + 8 + 31) // 32 * 32
+    centres = range(-h + 3, h - 3)                     # on-grid centre cells (DESIGN.md reading G10)
+    bases = sorted({(c - 3) & ~1 for c in centres})    # Python's & on negative ints is two's complement, like the kernel's
+    lo_b, hi_b = bases[0], bases[-1]
+    assert lo_b >= -h - 1 and hi_b + 7 <= h           # at most one cell outside on either side
+    lowest = (lo_b + h) * G + (lo_b + h)
+    highest = (hi_b + 7 + h) * G + (hi_b + 7 + h)
+    assert lowest >= -guard and highest < G * G + guard
