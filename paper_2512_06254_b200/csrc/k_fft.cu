@@ -1,0 +1,221 @@
+// k_fft.cu -- step a6 (+ a7), hand-written: the pruned inverse 2-D transform of the gridding grid
+// (PAPER.md:301 names the inverse FFT as the heaviest stage).
+//   F[m][n] = sum_{y, x} grid[y][x] exp(+2 pi i (x n + y m) / G)       (array indices; the grid is stored
+//   centred, which multiplies F by (-1)^(n + m): undone where the image is written, as in k_correct_crop)
+// Only the N columns n and N rows m the crop keeps are ever needed, and only 2-3 % of the grid is
+// non-zero.  Two kernels, both built on the shared-memory FFT of fft_smem.cuh:
+//   k_fft_rows   one CTA per grid row: the row is read THROUGH THE TILE MAP of the sparse clear (tiles
+//                the gridder did not mark are known to be zero and are not read: 25 MB instead of
+//                134 MB at config 2), transformed along x, and only the N needed columns are written
+//                to the workspace (a row without a marked tile writes zeros and skips the transform);
+//   k_fft_cols   one CTA per C adjacent needed columns: read strided (C x 8 B per row), transformed
+//                along y, and only the N needed rows leave the SM -- either as the finished image
+//                pixel Re F (-1)^(n+m) / (psi psi omega Wsum) (correction, crop and normalisation of
+//                step a7 fused: the transformed grid is never written back), or, for the Chebyshev
+//                moments of the 3-D mode, as complex values in place.
+// cuFFT needs G x G reads and writes in both passes, a separate crop kernel, and cannot skip zeros.
+// For G = 2^10 .. 2^13 with G >= 4N/3 and N a multiple of 16; other shapes stay on cuFFT.
+#include "fft_smem.cuh"
+#include "toi_internal.cuh"
+
+namespace toi {
+namespace {
+
+// Persistent CTAs (the twiddle tables are filled once per CTA): CTA b takes rows b, b + gridDim.x, ...
+template <int LOG2G>
+__global__ void __launch_bounds__((1 << LOG2G) / 16, LOG2G <= 12 ? 3 : 1)
+k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uint8_t *__restrict__ map, int N,
+           const float2 *__restrict__ tw)
+{
+    constexpr int G = 1 << LOG2G, T = G / 16;
+    extern __shared__ float2 s_dyn[];
+    float2 *const s_tab = s_dyn, *const s_seq = s_dyn + fft::kTabFloat2;
+    const int t = threadIdx.x, half = N >> 1;
+    fft::fill_tables<LOG2G>(s_tab, tw, t, T);
+    for (int y = blockIdx.x; y < G; y += gridDim.x) {
+        const uint8_t *mrow = map + (size_t)(y / kTileH) * tiles_per_row(G);
+        const float2 *src = grid + (size_t)y * G;
+        int any = 0;
+        __syncthreads();                         // the previous row's stores have read s_seq; the tables are filled
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int x = t + q * T;
+            float2 v = make_float2(0.0f, 0.0f);
+            if (__ldg(mrow + x / kTileW) != 0) {
+                v = __ldcs(src + x);             // read once: the clear zeroes it next
+                any = 1;
+            }
+            s_seq[fft::pad(x)] = v;
+        }
+        any = __syncthreads_or(any);
+        float2 *dst = work + (size_t)y * G;
+        if (!any) {                              // an all-zero row transforms to zeros
+            for (int n = t; n < half; n += T) {
+                dst[n] = make_float2(0.0f, 0.0f);
+                dst[G - half + n] = make_float2(0.0f, 0.0f);
+            }
+            continue;
+        }
+        fft::transform<LOG2G>(s_seq, t, s_tab, tw);
+        for (int n = t; n < half; n += T) {
+            dst[n] = s_seq[fft::pad(n)];
+            dst[G - half + n] = s_seq[fft::pad(G - half + n)];
+        }
+    }
+}
+
+// C columns per CTA pass, CT of them in flight at a time (CT groups of G / 16 threads); persistent CTAs.
+// Sequences sit kSkew float2 apart beyond their padded length, so that the C columns of one grid row
+// fall on different banks when a row segment is stored.
+constexpr int kSkew = 4;
+template <int LOG2G, int C, int CT, bool IMAGE>
+__global__ void __launch_bounds__(((1 << LOG2G) / 16) * CT)
+k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, const double *__restrict__ ipsi,
+           const SnapState *__restrict__ st, int apply_jacobian, float *__restrict__ image)
+{
+    constexpr int G = 1 << LOG2G, T = G / 16, NT = T * CT, SEQ = fft::padded(G) + kSkew;
+    constexpr int kPairs = C / 2, kLoads = (kPairs * G) / NT;      // float4 (two columns of a row) loads per thread
+    static_assert(C % 2 == 0 && (kPairs * G) % NT == 0, "column pairs must divide evenly among the threads");
+    extern __shared__ float2 s_dyn[];
+    float2 *const s_tab = s_dyn, *const s_seq = s_dyn + fft::kTabFloat2;     // [C][SEQ]
+    const int tid = threadIdx.x, half = N >> 1;
+    fft::fill_tables<LOG2G>(s_tab, tw, tid, NT);
+    const double wsum = st->wsum;
+    const bool ok = st->status == TOI_OK && wsum > 0.0;
+    const double inv_norm = ok ? 1.0 / ((apply_jacobian ? st->omega : 1.0) * wsum) : 0.0;
+    const int grp = tid / T, t = tid % T;
+    for (int first = blockIdx.x * C; first < N; first += gridDim.x * C) {
+        // my C columns: array indices n0 .. n0 + C - 1, inside [0, N/2) or [G - N/2, G)
+        const int n0 = first < half ? first : G - half + (first - half);
+        __syncthreads();                         // the previous pass has read s_seq; the tables are filled
+        // all loads first (16 bytes = two columns of one row each), then the shared-memory stores
+        float4 ld[kLoads];
+#pragma unroll
+        for (int u = 0; u < kLoads; ++u) {
+            const int idx = tid + u * NT, cp = idx % kPairs, y = idx / kPairs;
+            ld[u] = *reinterpret_cast<const float4 *>(work + (size_t)y * G + n0 + 2 * cp);
+        }
+#pragma unroll
+        for (int u = 0; u < kLoads; ++u) {
+            const int idx = tid + u * NT, cp = idx % kPairs, y = idx / kPairs;
+            s_seq[(2 * cp) * SEQ + fft::pad(y)] = make_float2(ld[u].x, ld[u].y);
+            s_seq[(2 * cp + 1) * SEQ + fft::pad(y)] = make_float2(ld[u].z, ld[u].w);
+        }
+        __syncthreads();
+#pragma unroll 1
+        for (int c = grp; c < C; c += CT) fft::transform<LOG2G>(s_seq + c * SEQ, t, s_tab, tw);
+        if (IMAGE) {
+            // step a7 fused: image[j][i] = Re F[m][n] (-1)^(n+m) / (psi(n) psi(m) omega Wsum), n = i - N/2, m = j - N/2
+            const int i0 = (n0 < half ? n0 : n0 - G) + half;     // image column of my first column
+            for (int idx = tid; idx < C * N; idx += NT) {
+                const int c = idx % C, j = idx / C;
+                const int m = j - half, i = i0 + c, n = i - half;
+                float out = 0.0f;
+                if (ok) {
+                    const float re = s_seq[c * SEQ + fft::pad(m < 0 ? m + G : m)].x;
+                    const float f = (float)(ipsi[i] * ipsi[j] * inv_norm);
+                    out = ((n + m) & 1) ? -(re * f) : re * f;
+                }
+                image[(size_t)j * N + i] = out;
+            }
+        } else {
+            // the complex transform, in place, for the rows the crop keeps (3-D mode: k_cheb_combine reads them)
+            for (int idx = tid; idx < C * N; idx += NT) {
+                const int c = idx % C, r = idx / C;
+                const int y = r < half ? r : G - N + r;
+                work[(size_t)y * G + n0 + c] = s_seq[c * SEQ + fft::pad(y)];
+            }
+        }
+    }
+}
+
+template <int LOG2G>
+void rows_launch(const float2 *grid, float2 *work, const uint8_t *map, int N, const float2 *tw, int n_sms,
+                 cudaStream_t stream)
+{
+    constexpr int G = 1 << LOG2G;
+    constexpr size_t smem = (size_t)(fft::kTabFloat2 + fft::padded(G)) * sizeof(float2);
+    static const cudaError_t once = cudaFuncSetAttribute(k_fft_rows<LOG2G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    (void)once;
+    int per_sm = (int)((220 * 1024) / smem);
+    if (per_sm * (G / 16) > 2048) per_sm = 2048 / (G / 16);
+    if (per_sm < 1) per_sm = 1;
+    int ctas = per_sm * n_sms;
+    if (ctas > G) ctas = G;
+    k_fft_rows<LOG2G><<<ctas, G / 16, smem, stream>>>(grid, work, map, N, tw);
+}
+
+template <int LOG2G, int C, int CT>
+void cols_launch(float2 *work, int N, const float2 *tw, const double *ipsi, const SnapState *st, int apply_jacobian,
+                 float *image, int n_sms, cudaStream_t stream)
+{
+    constexpr int G = 1 << LOG2G;
+    constexpr size_t smem = (size_t)(fft::kTabFloat2 + C * (fft::padded(G) + kSkew)) * sizeof(float2);
+    int per_sm = (int)((220 * 1024) / smem);
+    if (per_sm * (G / 16) * CT > 2048) per_sm = 2048 / ((G / 16) * CT);
+    if (per_sm < 1) per_sm = 1;
+    int ctas = per_sm * n_sms;
+    if (ctas > N / C) ctas = N / C;
+    if (image) {
+        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        (void)once;
+        k_fft_cols<LOG2G, C, CT, true><<<ctas, (G / 16) * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image);
+    } else {
+        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        (void)once;
+        k_fft_cols<LOG2G, C, CT, false><<<ctas, (G / 16) * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image);
+    }
+}
+
+int log2_exact(int G)
+{
+    for (int l = 0; l < 31; ++l)
+        if ((1 << l) == G) return l;
+    return -1;
+}
+
+}  // namespace
+
+// shapes the hand-written transform takes: G = 2^10 .. 2^13, pruned (4 N <= 3 G), N a multiple of 16
+bool fft_custom_supported(int N, int G)
+{
+    const int l = log2_exact(G);
+    return l >= 10 && l <= 13 && 4 * N <= 3 * G && N % 16 == 0;
+}
+
+// W^m = exp(+2 pi i m / G), m = 0 .. G - 1, computed in fp64
+void fft_twiddle_table(int G, float2 *host_out)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int m = 0; m < G; ++m) {
+        const double a = two_pi * (double)m / (double)G;
+        host_out[m] = make_float2((float)cos(a), (float)sin(a));
+    }
+}
+
+// pass 1: rows of `grid` (read through the tile map) -> needed columns of `work`
+void launch_fft_rows(int N, int G, const float2 *d_grid, float2 *d_work, const uint8_t *d_map, const float2 *d_tw,
+                     int n_sms, cudaStream_t stream)
+{
+    switch (log2_exact(G)) {
+    case 10: rows_launch<10>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    case 11: rows_launch<11>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    case 12: rows_launch<12>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    default: rows_launch<13>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    }
+}
+
+// pass 2: needed columns of `work`; d_image != nullptr: the finished image (step a7 fused), else the complex
+// values of the needed rows in place
+void launch_fft_cols(int N, int G, float2 *d_work, const float2 *d_tw, const double *d_ipsi, const SnapState *st,
+                     int apply_jacobian, float *d_image, int n_sms, cudaStream_t stream)
+{
+    switch (log2_exact(G)) {
+    case 10: cols_launch<10, 8, 8>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    case 11: cols_launch<11, 8, 4>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    case 12: cols_launch<12, 4, 2>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    default: cols_launch<13, 2, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    }
+}
+
+}  // namespace toi

@@ -259,6 +259,13 @@ inline size_t grid_guard(int G) { return ((size_t)G + 8 + 31) / 32 * 32; }
 void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                             float2 *d_grid, uint8_t *tiles, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
 void launch_clear_tiles(float2 *d_grid, float *d_density, int G, uint8_t *d_map, cudaStream_t stream);
+// hand-written pruned transform (k_fft.cu): rows through the tile map, then columns with the crop fused
+bool fft_custom_supported(int N, int G);
+void fft_twiddle_table(int G, float2 *host_out);
+void launch_fft_rows(int N, int G, const float2 *d_grid, float2 *d_work, const uint8_t *d_map, const float2 *d_tw,
+                     int n_sms, cudaStream_t stream);
+void launch_fft_cols(int N, int G, float2 *d_work, const float2 *d_tw, const double *d_ipsi, const SnapState *st,
+                     int apply_jacobian, float *d_image, int n_sms, cudaStream_t stream);
 void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s_min, double s_max, double *d_out,
                      cudaStream_t stream);
 size_t bessel_table_doubles(int K);

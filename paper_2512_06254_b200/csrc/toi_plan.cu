@@ -64,6 +64,8 @@ struct toi_plan {
 
     cufftHandle fft = 0, fft_cols = 0, fft_rows = 0;
     bool fft_ok = false, fft_pruned = false;
+    bool fft_custom = false;                             // k_fft.cu instead of cuFFT (+ k_correct_crop)
+    float2 *d_tw = nullptr;                              // its twiddle table, G entries
     cudaStream_t s_compute = nullptr, s_copy = nullptr, fft_stream = nullptr;
     cudaEvent_t ev[EV_COUNT] = {};
     cudaEvent_t ev_h2d_start[2] = {}, ev_h2d_done[2] = {}, ev_c_start[2] = {}, ev_c_done[2] = {}, ev_first = nullptr;
@@ -177,7 +179,7 @@ int free_plan(toi_plan *p)
     if (p->ev_first) cudaEventDestroy(p->ev_first);
     for (int k = 0; k < EV_COUNT; ++k)
         if (p->ev[k]) cudaEventDestroy(p->ev[k]);
-    cudaFree(p->d_grid_alloc); cudaFree(p->d_work); cudaFree(p->d_dens);
+    cudaFree(p->d_grid_alloc); cudaFree(p->d_work); cudaFree(p->d_dens); cudaFree(p->d_tw);
     cudaFree(p->d_tiles_grid);
     cudaFree(p->d_grid_keep); cudaFree(p->d_dens_keep);
     if (p->ev_done) cudaEventDestroy(p->ev_done);
@@ -226,14 +228,18 @@ uint8_t *gridder_tile_map(toi_plan *p, cudaStream_t stream, bool sliding)
     return nullptr;
 }
 
-// a6, first half + sparse clear: the first FFT pass reads the grid OUT OF PLACE into the workspace,
+// a6 + sparse clear (+ a7): the first transform pass reads the grid OUT OF PLACE into the workspace,
 // after which the tiles the gridder touched are zeroed again for the next snapshot (or pass); the
-// second FFT pass runs in place on the workspace.  Returns the number of launches through *launches.
-int transform_and_clear(toi_plan *p, cudaStream_t stream, bool clear_density, bool time_clear, int *launches)
+// second pass runs on the workspace.  d_image != nullptr: correction + crop + normalisation into that
+// image follow (fused into the second pass by the hand-written transform); nullptr: the complex
+// transform is left in the workspace (3-D mode).  `timed`: record the stage events of the 2-D path.
+int transform_and_clear(toi_plan *p, cudaStream_t stream, bool clear_density, bool timed, float *d_image, int *launches)
 {
     const Geometry &g = p->geo;
     cufftComplex *A = (cufftComplex *)p->d_grid, *F = (cufftComplex *)p->d_work;
-    if (p->fft_pruned) {
+    if (p->fft_custom) {
+        launch_fft_rows(g.N, g.G, p->d_grid, p->d_work, p->d_tiles_grid, p->d_tw, p->n_sms, stream);
+    } else if (p->fft_pruned) {
         // row transforms of all G rows (contiguous), then column transforms of only the N columns
         // the crop reads (columns n = -N/2..N/2-1 live at indices [0, N/2) and [G - N/2, G))
         if (cufftExecC2C(p->fft_rows, A, F, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
@@ -241,16 +247,27 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, bool clear_density, bo
         if (cufftExecC2C(p->fft, A, F, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
     }
     ++*launches;
-    if (time_clear) CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
     launch_clear_tiles(p->d_grid, clear_density ? p->d_dens : nullptr, g.G, p->d_tiles_grid, stream);
     ++*launches;
-    if (time_clear) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
+    if (p->fft_custom) {
+        launch_fft_cols(g.N, g.G, p->d_work, p->d_tw, p->d_ipsi, p->d_state, p->apply_jacobian, d_image, p->n_sms, stream);
+        ++*launches;
+        if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
+        return TOI_OK;
+    }
     if (p->fft_pruned) {
         cufftComplex *Fhi = F + (g.G - g.N / 2);
         if (cufftExecC2C(p->fft_cols, F, F, CUFFT_INVERSE) != CUFFT_SUCCESS ||
             cufftExecC2C(p->fft_cols, Fhi, Fhi, CUFFT_INVERSE) != CUFFT_SUCCESS)
             return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
         *launches += 2;
+    }
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
+    if (d_image) {
+        launch_correct_crop(g, p->d_work, p->d_ipsi, p->d_state, p->apply_jacobian, d_image, stream);
+        ++*launches;
     }
     return TOI_OK;
 }
@@ -291,15 +308,13 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
         CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
         if (uniform) CU_TRY(p, cudaMemcpyAsync(p->d_dens_keep, p->d_dens, GG * sizeof(float), cudaMemcpyDeviceToDevice, stream));
     }
-    // a6: inverse C2C FFT, grid -> workspace, with the sparse clear of the grid inside
-    rc = transform_and_clear(p, stream, uniform, true, &launches);
-    if (rc) return rc;
-    CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
-    // a7: correction + crop + normalisation into the image ring
+    // a6: inverse C2C FFT, grid -> workspace, with the sparse clear of the grid inside;
+    // a7: correction + crop + normalisation into the image ring (fused into the transform's second
+    // pass when the hand-written transform runs: ms_crop is then ~0 and ms_fft holds both)
     float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
     ++p->ring_pos;
-    launch_correct_crop(g, p->d_work, p->d_ipsi, p->d_state, p->apply_jacobian, img, stream);
-    ++launches;
+    rc = transform_and_clear(p, stream, uniform, true, img, &launches);
+    if (rc) return rc;
     CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
     CU_TRY(p, cudaEventRecord(p->ev_done, stream));
     CU_TRY(p, cudaGetLastError());
@@ -523,7 +538,14 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     // column pass is the expensive one (two kernels), so skipping G - N columns saves more than a
     // third of the FFT.  The skipped columns are left row-transformed only; nothing reads them.
     // Otherwise the plain 2-D plan.
-    if (4 * N <= 3 * G) {
+    if (fft_custom_supported(N, G)) {
+        // the hand-written pruned transform (k_fft.cu): no cuFFT plan at all
+        std::vector<float2> tw((size_t)G);
+        fft_twiddle_table(G, tw.data());
+        CREATE_TRY(cudaMalloc(&p->d_tw, (size_t)G * sizeof(float2)));
+        CREATE_TRY(cudaMemcpy(p->d_tw, tw.data(), (size_t)G * sizeof(float2), cudaMemcpyHostToDevice));
+        p->fft_custom = true;
+    } else if (4 * N <= 3 * G) {
         int n[1] = {G};
         if (cufftPlanMany(&p->fft_cols, 1, n, n, G, 1, n, G, 1, CUFFT_C2C, N / 2) != CUFFT_SUCCESS ||
             cufftPlanMany(&p->fft_rows, 1, n, n, 1, G, n, 1, G, CUFFT_C2C, G) != CUFFT_SUCCESS) {
@@ -735,7 +757,7 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
             }
             // first FFT pass out of place, sparse clear of the grid (and, after the last pass, of
             // the density map), second FFT pass on the workspace
-            rc = transform_and_clear(p, stream, uniform && last, false, &launches);
+            rc = transform_and_clear(p, stream, uniform && last, false, nullptr, &launches);
             if (rc) return rc;
             const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
             launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->d_work, p->d_ipsi, p->d_acc3,

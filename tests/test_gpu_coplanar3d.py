@@ -320,3 +320,34 @@ def test_3d_mode_at_config5_full_size_against_eq18():
           "(sampled expansion error %.3e); the 2-D image is off by %.3e" %
           (i3["n_slab"], i3["K"], phi_o, err, err / scale, eps, err2d))
     assert err <= (1.5 * eps + 2e-5) * scale
+
+
+def test_3d_mode_on_the_hand_written_transform():
+    """N = 512 (G = 1024): the Chebyshev moments go through k_fft_rows / k_fft_cols (complex output in
+    place) instead of cuFFT, which the N = 64 cases above use.  Sampled pixels against Eq. 18 itself, and
+    the whole image against the cuFFT-sized case's property that a planar array gives the 2-D image."""
+    snap = make_snapshot(seed=31, flags=True)
+    N, cell = 512, 25.0 / 3600.0                                 # same 3.6 deg field as the N = 64 cases
+    rc, V, omega, _ = oracle.plane_fit(snap["uvw_m"], snap["chan_freq_hz"])
+    assert rc == 0
+    r, z, wI = oracle_inputs(snap, V)
+    wsum = float(np.sum(wI))
+    img3, i3, info, img2 = run_gpu(snap, N, cell, 2, 16)
+    assert info["n_off_grid"] == 0 and info["n_gridded"] == z.size and abs(info["wsum"] - wsum) <= 2e-6 * wsum
+    rng = np.random.default_rng(77)
+    pi = np.concatenate([[N // 2, 0, N - 1, 0, N - 1], rng.integers(0, N, 60)])
+    pj = np.concatenate([[N // 2, 0, 0, N - 1, N - 1], rng.integers(0, N, 60)])
+    direct = o3.image_3d_direct_pixels(r, z, V, omega, N, cell, pi, pj, wsum=wsum)
+    got = img3[pj, pi]
+    assert np.array_equal(np.isnan(got), np.isnan(direct.real))
+    ok = ~np.isnan(got)
+    assert ok.sum() > 50
+    phi_o, _ = o3.phi_max_of(V, r[:, 2], N, cell)
+    eps = o3.sampled_error(phi_o / 2, 16)
+    scale = float(np.sum(np.abs(z))) / wsum
+    assert np.max(np.abs(got[ok] - direct.real[ok])) <= (1.5 * eps + 2e-5) * scale
+    planar = make_snapshot(seed=32, bump_m=0.0)
+    img3, i3, info, img2 = run_gpu(planar, N, cell, 0, 0)
+    ok = ~np.isnan(img3)
+    assert ok.mean() > 0.9
+    assert np.max(np.abs(img3[ok] - img2[ok])) <= 1e-5 * float(np.max(np.abs(img2)))
