@@ -81,6 +81,13 @@ struct toi_plan {
     // pinned host memory, Bessel table; the passes run on d_grid / d_work like the 2-D path
     float2 *d_acc3 = nullptr;
     double *d_r3 = nullptr, *h_r3 = nullptr, *d_jtab = nullptr;
+    // second lane of the 3-D mode (hand-written transform only): odd passes grid, transform and combine
+    // on their own grid / workspace / tile map on s_lane1, so that one pass's transform runs under the
+    // next pass's gridding; the gridders and the combinations of the two lanes are chained by events
+    float2 *d_grid1 = nullptr, *d_grid1_alloc = nullptr, *d_work1 = nullptr;
+    uint8_t *d_tiles1 = nullptr;
+    cudaStream_t s_lane1 = nullptr;
+    cudaEvent_t ev_lane_grid[2] = {}, ev_lane_comb[2] = {}, ev_lane_setup = nullptr;
     double s_min = 0, s_max = 0;
     cudaEvent_t ev3_a = nullptr, ev3_b = nullptr;
 
@@ -197,6 +204,14 @@ int free_plan(toi_plan *p)
     if (p->ev_tail) cudaEventDestroy(p->ev_tail);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
     cudaFree(p->d_acc3); cudaFree(p->d_r3); cudaFree(p->d_jtab);
+    if (p->s_lane1) cudaStreamSynchronize(p->s_lane1);
+    cudaFree(p->d_grid1_alloc); cudaFree(p->d_work1); cudaFree(p->d_tiles1);
+    for (int k = 0; k < 2; ++k) {
+        if (p->ev_lane_grid[k]) cudaEventDestroy(p->ev_lane_grid[k]);
+        if (p->ev_lane_comb[k]) cudaEventDestroy(p->ev_lane_comb[k]);
+    }
+    if (p->ev_lane_setup) cudaEventDestroy(p->ev_lane_setup);
+    if (p->s_lane1) cudaStreamDestroy(p->s_lane1);
     cudaFreeHost(p->h_r3);
     if (p->ev3_a) cudaEventDestroy(p->ev3_a);
     if (p->ev3_b) cudaEventDestroy(p->ev3_b);
@@ -221,10 +236,10 @@ int set_fft_stream(toi_plan *p, cudaStream_t stream)
 
 // The gridder marks the tiles it writes only when the channel scales are monotone (it bounds a
 // strip by its two end samples); otherwise, and for the strawman gridder, every tile is marked here.
-uint8_t *gridder_tile_map(toi_plan *p, cudaStream_t stream, bool sliding)
+uint8_t *gridder_tile_map(toi_plan *p, cudaStream_t stream, bool sliding, uint8_t *map)
 {
-    if (sliding && p->s_monotone) return p->d_tiles_grid;
-    cudaMemsetAsync(p->d_tiles_grid, 1, p->n_tiles, stream);
+    if (sliding && p->s_monotone) return map;
+    cudaMemsetAsync(map, 1, p->n_tiles, stream);
     return nullptr;
 }
 
@@ -233,12 +248,13 @@ uint8_t *gridder_tile_map(toi_plan *p, cudaStream_t stream, bool sliding)
 // second pass runs on the workspace.  d_image != nullptr: correction + crop + normalisation into that
 // image follow (fused into the second pass by the hand-written transform); nullptr: the complex
 // transform is left in the workspace (3-D mode).  `timed`: record the stage events of the 2-D path.
-int transform_and_clear(toi_plan *p, cudaStream_t stream, bool clear_density, bool timed, float *d_image, int *launches)
+int transform_and_clear(toi_plan *p, cudaStream_t stream, float2 *d_grid, uint8_t *d_tiles, float2 *d_work,
+                        bool clear_density, bool timed, float *d_image, int *launches)
 {
     const Geometry &g = p->geo;
-    cufftComplex *A = (cufftComplex *)p->d_grid, *F = (cufftComplex *)p->d_work;
+    cufftComplex *A = (cufftComplex *)d_grid, *F = (cufftComplex *)d_work;
     if (p->fft_custom) {
-        launch_fft_rows(g.N, g.G, p->d_grid, p->d_work, p->d_tiles_grid, p->d_tw, p->n_sms, stream);
+        launch_fft_rows(g.N, g.G, d_grid, d_work, d_tiles, p->d_tw, p->n_sms, stream);
     } else if (p->fft_pruned) {
         // row transforms of all G rows (contiguous), then column transforms of only the N columns
         // the crop reads (columns n = -N/2..N/2-1 live at indices [0, N/2) and [G - N/2, G))
@@ -248,11 +264,11 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, bool clear_density, bo
     }
     ++*launches;
     if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
-    launch_clear_tiles(p->d_grid, clear_density ? p->d_dens : nullptr, g.G, p->d_tiles_grid, stream);
+    launch_clear_tiles(d_grid, clear_density ? p->d_dens : nullptr, g.G, d_tiles, stream);
     ++*launches;
     if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
     if (p->fft_custom) {
-        launch_fft_cols(g.N, g.G, p->d_work, p->d_tw, p->d_ipsi, p->d_state, p->apply_jacobian, d_image, p->n_sms, stream);
+        launch_fft_cols(g.N, g.G, d_work, p->d_tw, p->d_ipsi, p->d_state, p->apply_jacobian, d_image, p->n_sms, stream);
         ++*launches;
         if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
         return TOI_OK;
@@ -266,7 +282,7 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, bool clear_density, bo
     }
     if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
     if (d_image) {
-        launch_correct_crop(g, p->d_work, p->d_ipsi, p->d_state, p->apply_jacobian, d_image, stream);
+        launch_correct_crop(g, d_work, p->d_ipsi, p->d_state, p->apply_jacobian, d_image, stream);
         ++*launches;
     }
     return TOI_OK;
@@ -297,7 +313,7 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     CU_TRY(p, cudaEventRecord(p->ev[EV_WEIGHT], stream));
     // a3 + a5: cell indices and gridding onto the zero grid
     const bool sliding = p->cfg.gridder != TOI_GRIDDER_ATOMIC;
-    uint8_t *tiles = gridder_tile_map(p, stream, sliding);
+    uint8_t *tiles = gridder_tile_map(p, stream, sliding, p->d_tiles_grid);
     if (sliding)
         launch_grid_pair8(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, stream);
     else
@@ -313,7 +329,7 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     // pass when the hand-written transform runs: ms_crop is then ~0 and ms_fft holds both)
     float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
     ++p->ring_pos;
-    rc = transform_and_clear(p, stream, uniform, true, img, &launches);
+    rc = transform_and_clear(p, stream, p->d_grid, p->d_tiles_grid, p->d_work, uniform, true, img, &launches);
     if (rc) return rc;
     CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
     CU_TRY(p, cudaEventRecord(p->ev_done, stream));
@@ -519,6 +535,20 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
         CREATE_TRY(cudaMallocHost(&p->h_r3, 2 * sizeof(double)));
         CREATE_TRY(cudaEventCreate(&p->ev3_a));
         CREATE_TRY(cudaEventCreate(&p->ev3_b));
+        if (fft_custom_supported(N, G) && cfg->gridder == TOI_GRIDDER_SLIDING) {
+            CREATE_TRY(cudaMalloc(&p->d_grid1_alloc, (GG + 2 * grid_guard(G)) * sizeof(float2)));
+            CREATE_TRY(cudaMemset(p->d_grid1_alloc, 0, (GG + 2 * grid_guard(G)) * sizeof(float2)));
+            p->d_grid1 = p->d_grid1_alloc + grid_guard(G);
+            CREATE_TRY(cudaMalloc(&p->d_work1, GG * sizeof(float2)));
+            CREATE_TRY(cudaMalloc(&p->d_tiles1, p->n_tiles));
+            CREATE_TRY(cudaMemset(p->d_tiles1, 0, p->n_tiles));
+            CREATE_TRY(cudaStreamCreateWithFlags(&p->s_lane1, cudaStreamNonBlocking));
+            for (int k = 0; k < 2; ++k) {
+                CREATE_TRY(cudaEventCreateWithFlags(&p->ev_lane_grid[k], cudaEventDisableTiming));
+                CREATE_TRY(cudaEventCreateWithFlags(&p->ev_lane_comb[k], cudaEventDisableTiming));
+            }
+            CREATE_TRY(cudaEventCreateWithFlags(&p->ev_lane_setup, cudaEventDisableTiming));
+        }
     }
     CREATE_TRY(cudaMalloc(&p->d_images, (size_t)p->ring_depth * N * N * sizeof(float)));
     if (cfg->input_location == TOI_MEM_HOST) {
@@ -740,32 +770,50 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     const double a_max = d > 0.0 ? 2.0 * 3.14159265358979323846 * d * t3_max * (1.0 + 1e-9) : 0.0;
     launch_bessel_table(K, a_max, p->d_jtab, stream);
     ++launches;
-    bool first = true;
-    for (int sp = 0; sp < slabs_run; ++sp) {
-        for (int k = 0; k < K; ++k) {
-            ChebArgs ca;
-            ca.p = sp; ca.k = k; ca.n_slab = n_slab; ca.r3_min = r3_min; ca.d = d;
-            ca.count = (k == 0 ? 1 : 0) | (k == 0 && sp == 0 ? 2 : 0);
-            const bool last = sp == slabs_run - 1 && k == K - 1;
-            CU_TRY(p, cudaMemsetAsync(&p->d_state->task_counter, 0, sizeof(unsigned int), stream));
-            uint8_t *tiles = gridder_tile_map(p, stream, true);
-            launch_grid_pair8_cheb(g, in, p->d_state, dens, p->d_grid, tiles, p->n_sms, ca, stream);
-            launches += tiles ? 2 : 3;
-            if (first && p->keep_grid) {
-                CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
-                if (uniform) CU_TRY(p, cudaMemcpyAsync(p->d_dens_keep, p->d_dens, GG * sizeof(float), cudaMemcpyDeviceToDevice, stream));
-            }
-            // first FFT pass out of place, sparse clear of the grid (and, after the last pass, of
-            // the density map), second FFT pass on the workspace
-            rc = transform_and_clear(p, stream, uniform && last, false, nullptr, &launches);
-            if (rc) return rc;
-            const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
-            launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->d_work, p->d_ipsi, p->d_acc3,
-                                first ? 1 : 0, stream);
-            ++launches;
-            first = false;
-        }
+    // Two lanes (when the second set of buffers exists): even passes on `stream`, odd passes on s_lane1,
+    // each on its own grid / tile map / workspace.  A pass's transform (shared-memory and DRAM bound)
+    // then runs under the next pass's gridding (issue bound).  What the passes share is kept in order by
+    // events: the task counter and the density map (gridder p + 1 waits for gridder p), the accumulator
+    // (combination p + 1 waits for combination p).
+    const bool two_lanes = p->d_grid1 != nullptr;
+    if (two_lanes) {
+        CU_TRY(p, cudaEventRecord(p->ev_lane_setup, stream));
+        CU_TRY(p, cudaStreamWaitEvent(p->s_lane1, p->ev_lane_setup, 0));
     }
+    const int n_passes = slabs_run * K;
+    for (int pass = 0; pass < n_passes; ++pass) {
+        const int sp = pass / K, k = pass % K;
+        const int L = two_lanes ? (pass & 1) : 0;
+        cudaStream_t sL = L ? p->s_lane1 : stream;
+        float2 *gridL = L ? p->d_grid1 : p->d_grid, *workL = L ? p->d_work1 : p->d_work;
+        uint8_t *mapL = L ? p->d_tiles1 : p->d_tiles_grid;
+        ChebArgs ca;
+        ca.p = sp; ca.k = k; ca.n_slab = n_slab; ca.r3_min = r3_min; ca.d = d;
+        ca.count = (k == 0 ? 1 : 0) | (pass == 0 ? 2 : 0);
+        const bool last = pass == n_passes - 1;
+        if (two_lanes && pass > 0) CU_TRY(p, cudaStreamWaitEvent(sL, p->ev_lane_grid[L ^ 1], 0));
+        CU_TRY(p, cudaMemsetAsync(&p->d_state->task_counter, 0, sizeof(unsigned int), sL));
+        uint8_t *tiles = gridder_tile_map(p, sL, true, mapL);
+        launch_grid_pair8_cheb(g, in, p->d_state, dens, gridL, tiles, p->n_sms, ca, sL);
+        launches += tiles ? 2 : 3;
+        if (two_lanes) CU_TRY(p, cudaEventRecord(p->ev_lane_grid[L], sL));
+        if (pass == 0 && p->keep_grid) {
+            CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, gridL, GG * sizeof(float2), cudaMemcpyDeviceToDevice, sL));
+            if (uniform) CU_TRY(p, cudaMemcpyAsync(p->d_dens_keep, p->d_dens, GG * sizeof(float), cudaMemcpyDeviceToDevice, sL));
+        }
+        // first transform pass out of place, sparse clear of the grid (and, after the last pass, of
+        // the density map), second transform pass on the workspace
+        rc = transform_and_clear(p, sL, gridL, mapL, workL, uniform && last, false, nullptr, &launches);
+        if (rc) return rc;
+        const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
+        if (two_lanes && pass > 0) CU_TRY(p, cudaStreamWaitEvent(sL, p->ev_lane_comb[L ^ 1], 0));
+        launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, workL, p->d_ipsi, p->d_acc3,
+                            pass == 0 ? 1 : 0, sL);
+        ++launches;
+        if (two_lanes) CU_TRY(p, cudaEventRecord(p->ev_lane_comb[L], sL));
+    }
+    // the last combination may sit on the other lane
+    if (two_lanes && n_passes > 0 && ((n_passes - 1) & 1)) CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_lane_comb[1], 0));
     launch_cheb_finish(g.N, beta, p->d_state, p->apply_jacobian, p->d_acc3, img, stream);
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev3_b, stream));
