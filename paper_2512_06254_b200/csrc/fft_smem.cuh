@@ -146,8 +146,17 @@ __device__ __forceinline__ void fill_tables(float2 *tab, const float2 *__restric
 // Contains two CTA-wide barriers: every thread of the CTA must call it the same number of times.
 // `tab`: the shared-memory twiddle rows of this stage (NS = 16, 256) or nullptr (NS = 1: no twiddles;
 // NS = 4096: looked up in the global table `tw`, consecutive threads consecutive entries).
-template <int R, int G, int NS>
-__device__ __forceinline__ void stage(float2 *s, int t, const float2 *tab, const float2 *__restrict__ tw)
+// `out`: where the results go -- SmemOut (back into the sequence, followed by a barrier) or a functor
+// out(index, value) of the caller's (the last stage of a pass can hand its results straight to global
+// memory: consecutive threads hold consecutive indices).
+struct SmemOut {
+    float2 *s;
+    static constexpr bool kShared = true;
+    __device__ __forceinline__ void operator()(int i, float2 v) const { s[pad(i)] = v; }
+};
+
+template <int R, int G, int NS, class Out>
+__device__ __forceinline__ void stage(float2 *s, int t, const float2 *tab, const float2 *__restrict__ tw, const Out &out)
 {
     constexpr int T = G / 16, B = 16 / R;
     float2 v[16];
@@ -179,23 +188,26 @@ __device__ __forceinline__ void stage(float2 *s, int t, const float2 *tab, const
         dft<R>(v + q * R);
         const int j0 = (j - k) * R + k;
 #pragma unroll
-        for (int r = 0; r < R; ++r) s[pad(j0 + r * NS)] = v[q * R + r];
+        for (int r = 0; r < R; ++r) out(j0 + r * NS, v[q * R + r]);
     }
-    __syncthreads();
+    if (Out::kShared) __syncthreads();
 }
 
-// The whole transform, in place: G = 2^LOG2G, 10 <= LOG2G <= 14.  `tab`: fill_tables' output.
-template <int LOG2G>
-__device__ __forceinline__ void transform(float2 *s, int t, const float2 *tab, const float2 *__restrict__ tw)
+// The whole transform: G = 2^LOG2G, 10 <= LOG2G <= 14.  `tab`: fill_tables' output.  The last stage's
+// results go to `out` (SmemOut{s}: in place).
+template <int LOG2G, class Out>
+__device__ __forceinline__ void transform(float2 *s, int t, const float2 *tab, const float2 *__restrict__ tw, const Out &out)
 {
     constexpr int G = 1 << LOG2G;
-    stage<16, G, 1>(s, t, nullptr, tw);
-    stage<16, G, 16>(s, t, tab, tw);
-    if constexpr (LOG2G == 10) stage<4, G, 256>(s, t, tab + 64, tw);
-    if constexpr (LOG2G == 11) stage<8, G, 256>(s, t, tab + 64, tw);
-    if constexpr (LOG2G >= 12) stage<16, G, 256>(s, t, tab + 64, tw);
-    if constexpr (LOG2G == 13) stage<2, G, 4096>(s, t, nullptr, tw);
-    if constexpr (LOG2G == 14) stage<4, G, 4096>(s, t, nullptr, tw);
+    const SmemOut in_place{s};
+    stage<16, G, 1>(s, t, nullptr, tw, in_place);
+    stage<16, G, 16>(s, t, tab, tw, in_place);
+    if constexpr (LOG2G == 10) stage<4, G, 256>(s, t, tab + 64, tw, out);
+    if constexpr (LOG2G == 11) stage<8, G, 256>(s, t, tab + 64, tw, out);
+    if constexpr (LOG2G == 12) stage<16, G, 256>(s, t, tab + 64, tw, out);
+    if constexpr (LOG2G >= 13) stage<16, G, 256>(s, t, tab + 64, tw, in_place);
+    if constexpr (LOG2G == 13) stage<2, G, 4096>(s, t, nullptr, tw, out);
+    if constexpr (LOG2G == 14) stage<4, G, 4096>(s, t, nullptr, tw, out);
 }
 
 }  // namespace fft

@@ -21,6 +21,17 @@
 namespace toi {
 namespace {
 
+// where the row pass's last stage puts its results: the needed columns of the workspace row
+struct ToWorkspace {
+    float2 *dst;
+    int half, G_;
+    static constexpr bool kShared = false;
+    __device__ __forceinline__ void operator()(int n, float2 v) const
+    {
+        if (n < half || n >= G_ - half) dst[n] = v;
+    }
+};
+
 // Persistent CTAs (the twiddle tables are filled once per CTA): CTA b takes rows b, b + gridDim.x, ...
 template <int LOG2G>
 __global__ void __launch_bounds__((1 << LOG2G) / 16, LOG2G <= 12 ? 3 : 1)
@@ -32,16 +43,22 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
     float2 *const s_tab = s_dyn, *const s_seq = s_dyn + fft::kTabFloat2;
     const int t = threadIdx.x, half = N >> 1;
     fft::fill_tables<LOG2G>(s_tab, tw, t, T);
+    static_assert(G / kTileW <= 64, "a row's tile marks are carried as one 64-bit mask");
     for (int y = blockIdx.x; y < G; y += gridDim.x) {
         const uint8_t *mrow = map + (size_t)(y / kTileH) * tiles_per_row(G);
         const float2 *src = grid + (size_t)y * G;
         int any = 0;
-        __syncthreads();                         // the previous row's stores have read s_seq; the tables are filled
+        // the marks of this row's G / 128 tiles as a bit mask (lane l looks at tiles l and l + 32)
+        const int lane = t & 31;
+        const unsigned m_lo = __ballot_sync(0xffffffffu, lane < G / kTileW && __ldg(mrow + lane) != 0);
+        const unsigned m_hi = G / kTileW > 32 ? __ballot_sync(0xffffffffu, lane + 32 < G / kTileW && __ldg(mrow + lane + 32) != 0) : 0u;
+        const unsigned long long marks = ((unsigned long long)m_hi << 32) | m_lo;
+        __syncthreads();                         // the previous row's last stage has read s_seq; the tables are filled
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             const int x = t + q * T;
             float2 v = make_float2(0.0f, 0.0f);
-            if (__ldg(mrow + x / kTileW) != 0) {
+            if ((marks >> (x / kTileW)) & 1ull) {
                 v = __ldcs(src + x);             // read once: the clear zeroes it next
                 any = 1;
             }
@@ -56,11 +73,9 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
             }
             continue;
         }
-        fft::transform<LOG2G>(s_seq, t, s_tab, tw);
-        for (int n = t; n < half; n += T) {
-            dst[n] = s_seq[fft::pad(n)];
-            dst[G - half + n] = s_seq[fft::pad(G - half + n)];
-        }
+        // the last stage hands its results straight to the workspace: only the needed columns, 8-byte
+        // stores from consecutive threads to consecutive addresses
+        fft::transform<LOG2G>(s_seq, t, s_tab, tw, ToWorkspace{dst, half, G});
     }
 }
 
@@ -103,7 +118,7 @@ k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, cons
         }
         __syncthreads();
 #pragma unroll 1
-        for (int c = grp; c < C; c += CT) fft::transform<LOG2G>(s_seq + c * SEQ, t, s_tab, tw);
+        for (int c = grp; c < C; c += CT) fft::transform<LOG2G>(s_seq + c * SEQ, t, s_tab, tw, fft::SmemOut{s_seq + c * SEQ});
         if (IMAGE) {
             // step a7 fused: image[j][i] = Re F[m][n] (-1)^(n+m) / (psi(n) psi(m) omega Wsum), n = i - N/2, m = j - N/2
             const int i0 = (n0 < half ? n0 : n0 - G) + half;     // image column of my first column
