@@ -25,44 +25,47 @@ namespace {
 struct ToWorkspace {
     float2 *dst;
     int half, G_;
-    static constexpr bool kShared = false;
-    __device__ __forceinline__ void operator()(int n, float2 v) const
+    __device__ __forceinline__ void operator()(int n, float2 *, float2 v) const
     {
         if (n < half || n >= G_ - half) dst[n] = v;
     }
 };
 
 // Persistent CTAs (the twiddle tables are filled once per CTA): CTA b takes rows b, b + gridDim.x, ...
-template <int LOG2G>
-__global__ void __launch_bounds__((1 << LOG2G) / 16, LOG2G <= 12 ? 3 : 1)
+// T threads per row, G / T elements each.
+template <int LOG2G, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB)
 k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uint8_t *__restrict__ map, int N,
            const float2 *__restrict__ tw)
 {
-    constexpr int G = 1 << LOG2G, T = G / 16;
+    using P = fft::Plan<LOG2G>;
+    constexpr int G = 1 << LOG2G, kTiles = G / kTileW;
     extern __shared__ float2 s_dyn[];
-    float2 *const s_tab = s_dyn, *const s_seq = s_dyn + fft::kTabFloat2;
+    float2 *const s_tab = s_dyn, *const s_seq = s_dyn + P::kTabFloat2;
     const int t = threadIdx.x, half = N >> 1;
     fft::fill_tables<LOG2G>(s_tab, tw, t, T);
-    static_assert(G / kTileW <= 64, "a row's tile marks are carried as one 64-bit mask");
+    static_assert(kTiles <= 128, "a row's tile marks are carried as two 64-bit masks");
     for (int y = blockIdx.x; y < G; y += gridDim.x) {
         const uint8_t *mrow = map + (size_t)(y / kTileH) * tiles_per_row(G);
         const float2 *src = grid + (size_t)y * G;
         int any = 0;
-        // the marks of this row's G / 128 tiles as a bit mask (lane l looks at tiles l and l + 32)
+        // the marks of this row's G / 128 tiles as bit masks (lane l looks at tiles l, l + 32, l + 64, l + 96)
         const int lane = t & 31;
-        const unsigned m_lo = __ballot_sync(0xffffffffu, lane < G / kTileW && __ldg(mrow + lane) != 0);
-        const unsigned m_hi = G / kTileW > 32 ? __ballot_sync(0xffffffffu, lane + 32 < G / kTileW && __ldg(mrow + lane + 32) != 0) : 0u;
-        const unsigned long long marks = ((unsigned long long)m_hi << 32) | m_lo;
+        unsigned m[4];
+#pragma unroll
+        for (int w = 0; w < 4; ++w)
+            m[w] = 32 * w < kTiles ? __ballot_sync(0xffffffffu, lane + 32 * w < kTiles && __ldg(mrow + lane + 32 * w) != 0) : 0u;
+        const unsigned long long marks_lo = ((unsigned long long)m[1] << 32) | m[0], marks_hi = ((unsigned long long)m[3] << 32) | m[2];
         __syncthreads();                         // the previous row's last stage has read s_seq; the tables are filled
 #pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            const int x = t + q * T;
+        for (int q = 0; q < G / T; ++q) {
+            const int x = t + q * T, tile = x / kTileW;
             float2 v = make_float2(0.0f, 0.0f);
-            if ((marks >> (x / kTileW)) & 1ull) {
+            if (((tile < 64 ? marks_lo : marks_hi) >> (tile & 63)) & 1ull) {
                 v = __ldcs(src + x);             // read once: the clear zeroes it next
                 any = 1;
             }
-            s_seq[fft::pad(x)] = v;
+            s_seq[fft::phys<LOG2G>(x)] = v;
         }
         any = __syncthreads_or(any);
         float2 *dst = work + (size_t)y * G;
@@ -75,24 +78,26 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
         }
         // the last stage hands its results straight to the workspace: only the needed columns, 8-byte
         // stores from consecutive threads to consecutive addresses
-        fft::transform<LOG2G>(s_seq, t, s_tab, tw, ToWorkspace{dst, half, G});
+        fft::transform<LOG2G, T>(s_seq, t, s_tab, ToWorkspace{dst, half, G});
     }
 }
 
-// C columns per CTA pass, CT of them in flight at a time (CT groups of G / 16 threads); persistent CTAs.
+// C columns per CTA pass, CT of them in flight at a time (CT groups of T threads); persistent CTAs.
 // Sequences sit kSkew float2 apart beyond their padded length, so that the C columns of one grid row
 // fall on different banks when a row segment is stored.
 constexpr int kSkew = 4;
-template <int LOG2G, int C, int CT, bool IMAGE>
-__global__ void __launch_bounds__(((1 << LOG2G) / 16) * CT)
+template <int LOG2G, int C, int CT, int T, bool IMAGE>
+__global__ void __launch_bounds__(T * CT)
 k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, const double *__restrict__ ipsi,
            const SnapState *__restrict__ st, int apply_jacobian, float *__restrict__ image)
 {
-    constexpr int G = 1 << LOG2G, T = G / 16, NT = T * CT, SEQ = fft::padded(G) + kSkew;
+    using P = fft::Plan<LOG2G>;
+    constexpr int G = 1 << LOG2G, NT = T * CT, SEQ = P::kPadded + kSkew;
     constexpr int kPairs = C / 2, kLoads = (kPairs * G) / NT;      // float4 (two columns of a row) loads per thread
-    static_assert(C % 2 == 0 && (kPairs * G) % NT == 0, "column pairs must divide evenly among the threads");
+    constexpr int kBatch = kLoads < 16 ? kLoads : 16;
+    static_assert(C % 2 == 0 && (kPairs * G) % NT == 0 && kLoads % kBatch == 0, "column pairs must divide evenly among the threads");
     extern __shared__ float2 s_dyn[];
-    float2 *const s_tab = s_dyn, *const s_seq = s_dyn + fft::kTabFloat2;     // [C][SEQ]
+    float2 *const s_tab = s_dyn, *const s_seq = s_dyn + P::kTabFloat2;       // [C][SEQ]
     const int tid = threadIdx.x, half = N >> 1;
     fft::fill_tables<LOG2G>(s_tab, tw, tid, NT);
     const double wsum = st->wsum;
@@ -103,22 +108,26 @@ k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, cons
         // my C columns: array indices n0 .. n0 + C - 1, inside [0, N/2) or [G - N/2, G)
         const int n0 = first < half ? first : G - half + (first - half);
         __syncthreads();                         // the previous pass has read s_seq; the tables are filled
-        // all loads first (16 bytes = two columns of one row each), then the shared-memory stores
-        float4 ld[kLoads];
+        // batches of loads (16 bytes = two columns of one row each), then their shared-memory stores
+#pragma unroll 1
+        for (int u0 = 0; u0 < kLoads; u0 += kBatch) {
+            float4 ld[kBatch];
 #pragma unroll
-        for (int u = 0; u < kLoads; ++u) {
-            const int idx = tid + u * NT, cp = idx % kPairs, y = idx / kPairs;
-            ld[u] = *reinterpret_cast<const float4 *>(work + (size_t)y * G + n0 + 2 * cp);
-        }
+            for (int u = 0; u < kBatch; ++u) {
+                const int idx = tid + (u0 + u) * NT, cp = idx % kPairs, y = idx / kPairs;
+                ld[u] = *reinterpret_cast<const float4 *>(work + (size_t)y * G + n0 + 2 * cp);
+            }
 #pragma unroll
-        for (int u = 0; u < kLoads; ++u) {
-            const int idx = tid + u * NT, cp = idx % kPairs, y = idx / kPairs;
-            s_seq[(2 * cp) * SEQ + fft::pad(y)] = make_float2(ld[u].x, ld[u].y);
-            s_seq[(2 * cp + 1) * SEQ + fft::pad(y)] = make_float2(ld[u].z, ld[u].w);
+            for (int u = 0; u < kBatch; ++u) {
+                const int idx = tid + (u0 + u) * NT, cp = idx % kPairs, y = idx / kPairs;
+                s_seq[(2 * cp) * SEQ + fft::phys<LOG2G>(y)] = make_float2(ld[u].x, ld[u].y);
+                s_seq[(2 * cp + 1) * SEQ + fft::phys<LOG2G>(y)] = make_float2(ld[u].z, ld[u].w);
+            }
         }
         __syncthreads();
 #pragma unroll 1
-        for (int c = grp; c < C; c += CT) fft::transform<LOG2G>(s_seq + c * SEQ, t, s_tab, tw, fft::SmemOut{s_seq + c * SEQ});
+        for (int c = grp; c < C; c += CT) fft::transform<LOG2G, T>(s_seq + c * SEQ, t, s_tab, fft::SmemOut{});
+        __syncthreads();                         // output k of column c now sits at phys_out(k)
         if (IMAGE) {
             // step a7 fused: image[j][i] = Re F[m][n] (-1)^(n+m) / (psi(n) psi(m) omega Wsum), n = i - N/2, m = j - N/2
             const int i0 = (n0 < half ? n0 : n0 - G) + half;     // image column of my first column
@@ -127,7 +136,7 @@ k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, cons
                 const int m = j - half, i = i0 + c, n = i - half;
                 float out = 0.0f;
                 if (ok) {
-                    const float re = s_seq[c * SEQ + fft::pad(m < 0 ? m + G : m)].x;
+                    const float re = s_seq[c * SEQ + fft::phys_out<LOG2G>(m < 0 ? m + G : m)].x;
                     const float f = (float)(ipsi[i] * ipsi[j] * inv_norm);
                     out = ((n + m) & 1) ? -(re * f) : re * f;
                 }
@@ -138,47 +147,48 @@ k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, cons
             for (int idx = tid; idx < C * N; idx += NT) {
                 const int c = idx % C, r = idx / C;
                 const int y = r < half ? r : G - N + r;
-                work[(size_t)y * G + n0 + c] = s_seq[c * SEQ + fft::pad(y)];
+                work[(size_t)y * G + n0 + c] = s_seq[c * SEQ + fft::phys_out<LOG2G>(y)];
             }
         }
     }
 }
 
-template <int LOG2G>
+template <int LOG2G, int T, int MINB>
 void rows_launch(const float2 *grid, float2 *work, const uint8_t *map, int N, const float2 *tw, int n_sms,
                  cudaStream_t stream)
 {
+    using P = fft::Plan<LOG2G>;
     constexpr int G = 1 << LOG2G;
-    constexpr size_t smem = (size_t)(fft::kTabFloat2 + fft::padded(G)) * sizeof(float2);
-    static const cudaError_t once = cudaFuncSetAttribute(k_fft_rows<LOG2G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    constexpr size_t smem = (size_t)(P::kTabFloat2 + P::kPadded) * sizeof(float2);
+    static const cudaError_t once = cudaFuncSetAttribute(k_fft_rows<LOG2G, T, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     (void)once;
-    int per_sm = (int)((220 * 1024) / smem);
-    if (per_sm * (G / 16) > 2048) per_sm = 2048 / (G / 16);
+    int per_sm = (int)((224 * 1024) / (smem + 1024));
+    if (per_sm > MINB) per_sm = MINB;
     if (per_sm < 1) per_sm = 1;
     int ctas = per_sm * n_sms;
     if (ctas > G) ctas = G;
-    k_fft_rows<LOG2G><<<ctas, G / 16, smem, stream>>>(grid, work, map, N, tw);
+    k_fft_rows<LOG2G, T, MINB><<<ctas, T, smem, stream>>>(grid, work, map, N, tw);
 }
 
-template <int LOG2G, int C, int CT>
+template <int LOG2G, int C, int CT, int T>
 void cols_launch(float2 *work, int N, const float2 *tw, const double *ipsi, const SnapState *st, int apply_jacobian,
                  float *image, int n_sms, cudaStream_t stream)
 {
-    constexpr int G = 1 << LOG2G;
-    constexpr size_t smem = (size_t)(fft::kTabFloat2 + C * (fft::padded(G) + kSkew)) * sizeof(float2);
-    int per_sm = (int)((220 * 1024) / smem);
-    if (per_sm * (G / 16) * CT > 2048) per_sm = 2048 / ((G / 16) * CT);
+    using P = fft::Plan<LOG2G>;
+    constexpr size_t smem = (size_t)(P::kTabFloat2 + C * (P::kPadded + kSkew)) * sizeof(float2);
+    int per_sm = (int)((224 * 1024) / (smem + 1024));
+    if (per_sm * T * CT > 1024) per_sm = 1024 / (T * CT);
     if (per_sm < 1) per_sm = 1;
     int ctas = per_sm * n_sms;
     if (ctas > N / C) ctas = N / C;
     if (image) {
-        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        k_fft_cols<LOG2G, C, CT, true><<<ctas, (G / 16) * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image);
+        k_fft_cols<LOG2G, C, CT, T, true><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image);
     } else {
-        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        k_fft_cols<LOG2G, C, CT, false><<<ctas, (G / 16) * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image);
+        k_fft_cols<LOG2G, C, CT, T, false><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image);
     }
 }
 
@@ -213,10 +223,11 @@ void launch_fft_rows(int N, int G, const float2 *d_grid, float2 *d_work, const u
                      int n_sms, cudaStream_t stream)
 {
     switch (log2_exact(G)) {
-    case 10: rows_launch<10>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
-    case 11: rows_launch<11>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
-    case 12: rows_launch<12>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
-    default: rows_launch<13>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    case 10: rows_launch<10, 64, 8>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    case 11: rows_launch<11, 128, 4>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    case 12: rows_launch<12, 256, 3>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    case 13: rows_launch<13, 256, 2>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
+    default: rows_launch<14, 512, 1>(d_grid, d_work, d_map, N, d_tw, n_sms, stream); break;
     }
 }
 
@@ -226,10 +237,10 @@ void launch_fft_cols(int N, int G, float2 *d_work, const float2 *d_tw, const dou
                      int apply_jacobian, float *d_image, int n_sms, cudaStream_t stream)
 {
     switch (log2_exact(G)) {
-    case 10: cols_launch<10, 8, 8>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
-    case 11: cols_launch<11, 8, 4>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
-    case 12: cols_launch<12, 4, 2>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
-    default: cols_launch<13, 2, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    case 10: cols_launch<10, 8, 8, 64>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    case 11: cols_launch<11, 8, 4, 128>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    case 12: cols_launch<12, 4, 2, 256>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    default: cols_launch<13, 2, 2, 256>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
     }
 }
 
