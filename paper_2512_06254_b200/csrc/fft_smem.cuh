@@ -14,7 +14,7 @@
 // consecutive k, so a pass can write them straight to global memory in natural order.
 // Arithmetic: packed fp32 pairs (sm_100a FADD2 / FMUL2 / FFMA2: a complex add, or half a complex
 // multiply, per instruction; the multiplication by +-i is an operand modifier).
-// Padding: one element per 16, plus `delta` per block of G/16 so that the block stride is 1 mod 16:
+// Padding: one element per 16, plus one per block of G/16 so that the block stride is odd:
 // stage C's half-warp (16 different k1) then falls on 16 different bank pairs.
 // Twiddles: W^m = exp(+2 pi i m / G) from a table of G float2 computed in fp64 on the host; per
 // butterfly the powers w, w^2, w^4, w^8 (, w^16) of its base twiddle are looked up in per-stage tables
@@ -169,8 +169,9 @@ struct Plan {
     static constexpr int R3 = G / (16 * R2);                 // 4, 8, 16, 32, 32
     static constexpr int L1 = G / 16;                        // block length after stage A
     static constexpr int S2 = L1 / R2;                       // stride of stage B = number of its base twiddles
-    static constexpr int kDelta = (17 - (L1 + L1 / 16) % 16) % 16;
-    static constexpr int L1p = L1 + L1 / 16 + kDelta;        // padded block stride, 1 mod 16
+    static constexpr int kDelta = 1;
+    static constexpr int L1p = L1 + L1 / 16 + kDelta;        // padded block stride, odd
+    static_assert(L1p % 2 == 1, "block stride must be odd");
     static constexpr int kPadded = 16 * L1p;                 // float2 per sequence
     static constexpr int kTabBWidth = R2 == 32 ? 8 : 4;      // powers stored per row of stage B's table
     static constexpr int kTabA = L1 * 4, kTabB = S2 * kTabBWidth;

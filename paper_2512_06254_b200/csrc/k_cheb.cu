@@ -91,7 +91,7 @@ __device__ __forceinline__ double bessel_lookup(const double *__restrict__ row, 
 
 __global__ void __launch_bounds__(256)
 k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, int k, double r3_p, double d_r3,
-               const double *__restrict__ jrow, double a_max, const float2 *__restrict__ F,
+               const double *__restrict__ jrow, double a_max, const float2 *__restrict__ F, int compact,
                const double *__restrict__ ipsi, float2 *__restrict__ acc, int first)
 {
     const int i = blockIdx.x * 32 + (threadIdx.x & 31);
@@ -116,9 +116,10 @@ k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, 
         case 2: wr = -cp; wi = -sp; break;
         default: wr = sp; wi = -cp; break;
         }
-        // the moment at this pixel: cuFFT's unshifted output, (-1)^(n+m) of the centred grid, 1/(psi psi)
+        // the moment at this pixel: the transform's unshifted output (compact: already cropped to [j][i]),
+        // (-1)^(n+m) of the centred grid, 1/(psi psi)
         const int n = i - (N >> 1), m = j - (N >> 1);
-        const float2 f = __ldg(F + (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n));
+        const float2 f = __ldg(F + (compact ? o : (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n)));
         double c = ipsi[i] * ipsi[j] * ck;
         if ((n + m) & 1) c = -c;
         wr *= c; wi *= c;
@@ -163,12 +164,12 @@ void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream
 }
 
 void launch_cheb_combine(const Geometry &g, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
-                         const double *d_tab, double a_max, const float2 *d_F, const double *d_ipsi, float2 *d_acc,
-                         int first, cudaStream_t stream)
+                         const double *d_tab, double a_max, const float2 *d_F, int compact, const double *d_ipsi,
+                         float2 *d_acc, int first, cudaStream_t stream)
 {
     dim3 grid((g.N + 31) / 32, (g.N + 7) / 8);
     k_cheb_combine<<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k, r3_p, d_r3, d_tab + (size_t)k * (kJTab + 3),
-                                             a_max, d_F, d_ipsi, d_acc, first);
+                                             a_max, d_F, compact, d_ipsi, d_acc, first);
 }
 
 void launch_cheb_finish(int N, double beta_rad, const SnapState *st, int apply_jacobian, const float2 *d_acc,

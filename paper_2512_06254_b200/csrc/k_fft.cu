@@ -21,13 +21,25 @@
 namespace toi {
 namespace {
 
-// where the row pass's last stage puts its results: the needed columns of the workspace row
+// Workspace layout between the passes: only the N needed columns, in blocks of CB columns,
+//   work[(n' / CB) G CB + y CB + n' % CB],  n' = n for n < N/2, n - (G - N) for n >= G - N/2
+// so that the column pass reads the CB columns of a block as ONE contiguous run of G CB float2 (a
+// strided read of 32-byte row segments opens a DRAM page per segment and ran at a fifth of the
+// bandwidth); the scatter is on the write side, where nothing waits for it and L2 merges the
+// segments of neighbouring rows.  CB >= 4: the row pass writes whole 32-byte sectors.
+__host__ __device__ constexpr int cols_block(int log2g) { return log2g <= 11 ? 8 : 4; }
+
+// where the row pass's last stage puts its results
+template <int LOG2G>
 struct ToWorkspace {
-    float2 *dst;
-    int half, G_;
+    float2 *dst;                                 // work + y CB
+    int half, N_;
     __device__ __forceinline__ void operator()(int n, float2 *, float2 v) const
     {
-        if (n < half || n >= G_ - half) dst[n] = v;
+        constexpr int G = 1 << LOG2G, CB = cols_block(LOG2G);
+        const unsigned np = n < half ? n : n - (G - N_);
+        // 32-bit element index: G N < 2^31
+        if (n < half || n >= G - half) dst[(np / CB) * (unsigned)(G * CB) + np % CB] = v;
     }
 };
 
@@ -68,34 +80,38 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
             s_seq[fft::phys<LOG2G>(x)] = v;
         }
         any = __syncthreads_or(any);
-        float2 *dst = work + (size_t)y * G;
+        const ToWorkspace<LOG2G> to_work{work + (size_t)y * cols_block(LOG2G), half, N};
         if (!any) {                              // an all-zero row transforms to zeros
             for (int n = t; n < half; n += T) {
-                dst[n] = make_float2(0.0f, 0.0f);
-                dst[G - half + n] = make_float2(0.0f, 0.0f);
+                to_work(n, nullptr, make_float2(0.0f, 0.0f));
+                to_work(G - half + n, nullptr, make_float2(0.0f, 0.0f));
             }
             continue;
         }
         // the last stage hands its results straight to the workspace: only the needed columns, 8-byte
         // stores from consecutive threads to consecutive addresses
-        fft::transform<LOG2G, T>(s_seq, t, s_tab, ToWorkspace{dst, half, G});
+        fft::transform<LOG2G, T>(s_seq, t, s_tab, to_work);
     }
 }
 
-// C columns per CTA pass, CT of them in flight at a time (CT groups of T threads); persistent CTAs.
+// C columns (a part of a block of CB) per CTA pass, CT of them in flight at a time (CT groups of T threads);
+// persistent CTAs, CTA b takes parts b, b + gridDim.x, ... so that the parts of a block are read at about
+// the same time (the block's sectors then come from L2 for all but the first).
 // Sequences sit kSkew float2 apart beyond their padded length, so that the C columns of one grid row
 // fall on different banks when a row segment is stored.
 constexpr int kSkew = 4;
 template <int LOG2G, int C, int CT, int T, bool IMAGE>
 __global__ void __launch_bounds__(T * CT)
-k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, const double *__restrict__ ipsi,
-           const SnapState *__restrict__ st, int apply_jacobian, float *__restrict__ image)
+k_fft_cols(const float2 *__restrict__ work, int N, const float2 *__restrict__ tw, const double *__restrict__ ipsi,
+           const SnapState *__restrict__ st, int apply_jacobian, float *__restrict__ image, float2 *__restrict__ moment)
 {
     using P = fft::Plan<LOG2G>;
+    constexpr int CB = cols_block(LOG2G);
     constexpr int G = 1 << LOG2G, NT = T * CT, SEQ = P::kPadded + kSkew;
-    constexpr int kPairs = C / 2, kLoads = (kPairs * G) / NT;      // float4 (two columns of a row) loads per thread
+    constexpr int kW = C >= 2 ? 2 : 1;                   // float2 per load
+    constexpr int kLoads = (C * G / kW) / NT;            // loads per thread
     constexpr int kBatch = kLoads < 16 ? kLoads : 16;
-    static_assert(C % 2 == 0 && (kPairs * G) % NT == 0 && kLoads % kBatch == 0, "column pairs must divide evenly among the threads");
+    static_assert(CB % C == 0 && (C * G / kW) % NT == 0 && kLoads % kBatch == 0 && C % CT == 0, "a part must divide evenly among the threads");
     extern __shared__ float2 s_dyn[];
     float2 *const s_tab = s_dyn, *const s_seq = s_dyn + P::kTabFloat2;       // [C][SEQ]
     const int tid = threadIdx.x, half = N >> 1;
@@ -107,21 +123,30 @@ k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, cons
     for (int first = blockIdx.x * C; first < N; first += gridDim.x * C) {
         // my C columns: array indices n0 .. n0 + C - 1, inside [0, N/2) or [G - N/2, G)
         const int n0 = first < half ? first : G - half + (first - half);
+        const float2 *src = work + (size_t)(first / CB) * ((size_t)G * CB) + first % CB;
         __syncthreads();                         // the previous pass has read s_seq; the tables are filled
-        // batches of loads (16 bytes = two columns of one row each), then their shared-memory stores
+        // batches of loads, then their shared-memory stores
 #pragma unroll 1
         for (int u0 = 0; u0 < kLoads; u0 += kBatch) {
-            float4 ld[kBatch];
+            if constexpr (kW == 2) {
+                float4 ld[kBatch];
 #pragma unroll
-            for (int u = 0; u < kBatch; ++u) {
-                const int idx = tid + (u0 + u) * NT, cp = idx % kPairs, y = idx / kPairs;
-                ld[u] = *reinterpret_cast<const float4 *>(work + (size_t)y * G + n0 + 2 * cp);
-            }
+                for (int u = 0; u < kBatch; ++u) {
+                    const int idx = tid + (u0 + u) * NT, cp = idx % (C / 2), y = idx / (C / 2);
+                    ld[u] = __ldcs(reinterpret_cast<const float4 *>(src + (size_t)y * CB + 2 * cp));
+                }
 #pragma unroll
-            for (int u = 0; u < kBatch; ++u) {
-                const int idx = tid + (u0 + u) * NT, cp = idx % kPairs, y = idx / kPairs;
-                s_seq[(2 * cp) * SEQ + fft::phys<LOG2G>(y)] = make_float2(ld[u].x, ld[u].y);
-                s_seq[(2 * cp + 1) * SEQ + fft::phys<LOG2G>(y)] = make_float2(ld[u].z, ld[u].w);
+                for (int u = 0; u < kBatch; ++u) {
+                    const int idx = tid + (u0 + u) * NT, cp = idx % (C / 2), y = idx / (C / 2);
+                    s_seq[(2 * cp) * SEQ + fft::phys<LOG2G>(y)] = make_float2(ld[u].x, ld[u].y);
+                    s_seq[(2 * cp + 1) * SEQ + fft::phys<LOG2G>(y)] = make_float2(ld[u].z, ld[u].w);
+                }
+            } else {
+                float2 ld[kBatch];
+#pragma unroll
+                for (int u = 0; u < kBatch; ++u) ld[u] = __ldcs(src + (size_t)(tid + (u0 + u) * NT) * CB);
+#pragma unroll
+                for (int u = 0; u < kBatch; ++u) s_seq[fft::phys<LOG2G>(tid + (u0 + u) * NT)] = ld[u];
             }
         }
         __syncthreads();
@@ -143,11 +168,12 @@ k_fft_cols(float2 *__restrict__ work, int N, const float2 *__restrict__ tw, cons
                 image[(size_t)j * N + i] = out;
             }
         } else {
-            // the complex transform, in place, for the rows the crop keeps (3-D mode: k_cheb_combine reads them)
+            // the complex transform of the pixels the crop keeps, moment[j][i] = F[m][n] (3-D mode: k_cheb_combine reads it)
+            const int i0 = (n0 < half ? n0 : n0 - G) + half;
             for (int idx = tid; idx < C * N; idx += NT) {
-                const int c = idx % C, r = idx / C;
-                const int y = r < half ? r : G - N + r;
-                work[(size_t)y * G + n0 + c] = s_seq[c * SEQ + fft::phys_out<LOG2G>(y)];
+                const int c = idx % C, j = idx / C;
+                const int m = j - half;
+                moment[(size_t)j * N + i0 + c] = s_seq[c * SEQ + fft::phys_out<LOG2G>(m < 0 ? m + G : m)];
             }
         }
     }
@@ -171,8 +197,8 @@ void rows_launch(const float2 *grid, float2 *work, const uint8_t *map, int N, co
 }
 
 template <int LOG2G, int C, int CT, int T>
-void cols_launch(float2 *work, int N, const float2 *tw, const double *ipsi, const SnapState *st, int apply_jacobian,
-                 float *image, int n_sms, cudaStream_t stream)
+void cols_launch(const float2 *work, int N, const float2 *tw, const double *ipsi, const SnapState *st, int apply_jacobian,
+                 float *image, float2 *moment, int n_sms, cudaStream_t stream)
 {
     using P = fft::Plan<LOG2G>;
     constexpr size_t smem = (size_t)(P::kTabFloat2 + C * (P::kPadded + kSkew)) * sizeof(float2);
@@ -184,11 +210,11 @@ void cols_launch(float2 *work, int N, const float2 *tw, const double *ipsi, cons
     if (image) {
         static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        k_fft_cols<LOG2G, C, CT, T, true><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image);
+        k_fft_cols<LOG2G, C, CT, T, true><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image, moment);
     } else {
         static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        k_fft_cols<LOG2G, C, CT, T, false><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image);
+        k_fft_cols<LOG2G, C, CT, T, false><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image, moment);
     }
 }
 
@@ -201,11 +227,11 @@ int log2_exact(int G)
 
 }  // namespace
 
-// shapes the hand-written transform takes: G = 2^10 .. 2^13, pruned (4 N <= 3 G), N a multiple of 16
+// shapes the hand-written transform takes: G = 2^10 .. 2^14, pruned (4 N <= 3 G), N a multiple of 16
 bool fft_custom_supported(int N, int G)
 {
     const int l = log2_exact(G);
-    return l >= 10 && l <= 13 && 4 * N <= 3 * G && N % 16 == 0;
+    return l >= 10 && l <= 14 && 4 * N <= 3 * G && N % 16 == 0;
 }
 
 // W^m = exp(+2 pi i m / G), m = 0 .. G - 1, computed in fp64
@@ -231,16 +257,17 @@ void launch_fft_rows(int N, int G, const float2 *d_grid, float2 *d_work, const u
     }
 }
 
-// pass 2: needed columns of `work`; d_image != nullptr: the finished image (step a7 fused), else the complex
-// values of the needed rows in place
-void launch_fft_cols(int N, int G, float2 *d_work, const float2 *d_tw, const double *d_ipsi, const SnapState *st,
-                     int apply_jacobian, float *d_image, int n_sms, cudaStream_t stream)
+// pass 2: the needed columns of `work`; d_image != nullptr: the finished image (step a7 fused), else the
+// complex values of the N x N pixels the crop keeps into d_moment[j][i]
+void launch_fft_cols(int N, int G, const float2 *d_work, const float2 *d_tw, const double *d_ipsi, const SnapState *st,
+                     int apply_jacobian, float *d_image, float2 *d_moment, int n_sms, cudaStream_t stream)
 {
     switch (log2_exact(G)) {
-    case 10: cols_launch<10, 8, 8, 64>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
-    case 11: cols_launch<11, 8, 4, 128>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
-    case 12: cols_launch<12, 4, 2, 256>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
-    default: cols_launch<13, 2, 2, 256>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, n_sms, stream); break;
+    case 10: cols_launch<10, 8, 8, 64>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    case 11: cols_launch<11, 8, 4, 128>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    case 12: cols_launch<12, 4, 4, 128>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    case 13: cols_launch<13, 2, 2, 128>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    default: cols_launch<14, 1, 1, 512>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
     }
 }
 

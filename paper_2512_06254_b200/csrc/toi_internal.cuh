@@ -264,15 +264,15 @@ bool fft_custom_supported(int N, int G);
 void fft_twiddle_table(int G, float2 *host_out);
 void launch_fft_rows(int N, int G, const float2 *d_grid, float2 *d_work, const uint8_t *d_map, const float2 *d_tw,
                      int n_sms, cudaStream_t stream);
-void launch_fft_cols(int N, int G, float2 *d_work, const float2 *d_tw, const double *d_ipsi, const SnapState *st,
-                     int apply_jacobian, float *d_image, int n_sms, cudaStream_t stream);
+void launch_fft_cols(int N, int G, const float2 *d_work, const float2 *d_tw, const double *d_ipsi, const SnapState *st,
+                     int apply_jacobian, float *d_image, float2 *d_moment, int n_sms, cudaStream_t stream);
 void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s_min, double s_max, double *d_out,
                      cudaStream_t stream);
 size_t bessel_table_doubles(int K);
 void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream);
 void launch_cheb_combine(const Geometry &g, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
-                         const double *d_tab, double a_max, const float2 *d_F, const double *d_ipsi, float2 *d_acc,
-                         int first, cudaStream_t stream);
+                         const double *d_tab, double a_max, const float2 *d_F, int compact, const double *d_ipsi,
+                         float2 *d_acc, int first, cudaStream_t stream);
 void launch_cheb_finish(int N, double beta_rad, const SnapState *st, int apply_jacobian, const float2 *d_acc,
                         float *d_image, cudaStream_t stream);
 void launch_correct_crop(const Geometry &g, const float2 *d_F, const double *d_ipsi, const SnapState *st,

@@ -66,6 +66,7 @@ struct toi_plan {
     bool fft_ok = false, fft_pruned = false;
     bool fft_custom = false;                             // k_fft.cu instead of cuFFT (+ k_correct_crop)
     float2 *d_tw = nullptr;                              // its twiddle table, G entries
+    float2 *d_moment[2] = {nullptr, nullptr};            // 3-D mode: the cropped complex transform [N][N] of a pass, per lane
     cudaStream_t s_compute = nullptr, s_copy = nullptr, fft_stream = nullptr;
     cudaEvent_t ev[EV_COUNT] = {};
     cudaEvent_t ev_h2d_start[2] = {}, ev_h2d_done[2] = {}, ev_c_start[2] = {}, ev_c_done[2] = {}, ev_first = nullptr;
@@ -187,6 +188,7 @@ int free_plan(toi_plan *p)
     for (int k = 0; k < EV_COUNT; ++k)
         if (p->ev[k]) cudaEventDestroy(p->ev[k]);
     cudaFree(p->d_grid_alloc); cudaFree(p->d_work); cudaFree(p->d_dens); cudaFree(p->d_tw);
+    cudaFree(p->d_moment[0]); cudaFree(p->d_moment[1]);
     cudaFree(p->d_tiles_grid);
     cudaFree(p->d_grid_keep); cudaFree(p->d_dens_keep);
     if (p->ev_done) cudaEventDestroy(p->ev_done);
@@ -246,10 +248,11 @@ uint8_t *gridder_tile_map(toi_plan *p, cudaStream_t stream, bool sliding, uint8_
 // a6 + sparse clear (+ a7): the first transform pass reads the grid OUT OF PLACE into the workspace,
 // after which the tiles the gridder touched are zeroed again for the next snapshot (or pass); the
 // second pass runs on the workspace.  d_image != nullptr: correction + crop + normalisation into that
-// image follow (fused into the second pass by the hand-written transform); nullptr: the complex
-// transform is left in the workspace (3-D mode).  `timed`: record the stage events of the 2-D path.
+// image follow (fused into the second pass by the hand-written transform); nullptr (3-D mode): the
+// complex transform is left in the workspace (cuFFT) or, cropped, in d_moment[lane] (hand-written
+// transform).  `timed`: record the stage events of the 2-D path.
 int transform_and_clear(toi_plan *p, cudaStream_t stream, float2 *d_grid, uint8_t *d_tiles, float2 *d_work,
-                        bool clear_density, bool timed, float *d_image, int *launches)
+                        bool clear_density, bool timed, float *d_image, int lane, int *launches)
 {
     const Geometry &g = p->geo;
     cufftComplex *A = (cufftComplex *)d_grid, *F = (cufftComplex *)d_work;
@@ -268,7 +271,8 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, float2 *d_grid, uint8_
     ++*launches;
     if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
     if (p->fft_custom) {
-        launch_fft_cols(g.N, g.G, d_work, p->d_tw, p->d_ipsi, p->d_state, p->apply_jacobian, d_image, p->n_sms, stream);
+        launch_fft_cols(g.N, g.G, d_work, p->d_tw, p->d_ipsi, p->d_state, p->apply_jacobian, d_image,
+                        d_image ? nullptr : p->d_moment[lane], p->n_sms, stream);
         ++*launches;
         if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
         return TOI_OK;
@@ -329,7 +333,7 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     // pass when the hand-written transform runs: ms_crop is then ~0 and ms_fft holds both)
     float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
     ++p->ring_pos;
-    rc = transform_and_clear(p, stream, p->d_grid, p->d_tiles_grid, p->d_work, uniform, true, img, &launches);
+    rc = transform_and_clear(p, stream, p->d_grid, p->d_tiles_grid, p->d_work, uniform, true, img, 0, &launches);
     if (rc) return rc;
     CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
     CU_TRY(p, cudaEventRecord(p->ev_done, stream));
@@ -540,6 +544,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
             CREATE_TRY(cudaMemset(p->d_grid1_alloc, 0, (GG + 2 * grid_guard(G)) * sizeof(float2)));
             p->d_grid1 = p->d_grid1_alloc + grid_guard(G);
             CREATE_TRY(cudaMalloc(&p->d_work1, GG * sizeof(float2)));
+            CREATE_TRY(cudaMalloc(&p->d_moment[1], (size_t)N * N * sizeof(float2)));
             CREATE_TRY(cudaMalloc(&p->d_tiles1, p->n_tiles));
             CREATE_TRY(cudaMemset(p->d_tiles1, 0, p->n_tiles));
             CREATE_TRY(cudaStreamCreateWithFlags(&p->s_lane1, cudaStreamNonBlocking));
@@ -574,6 +579,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
         fft_twiddle_table(G, tw.data());
         CREATE_TRY(cudaMalloc(&p->d_tw, (size_t)G * sizeof(float2)));
         CREATE_TRY(cudaMemcpy(p->d_tw, tw.data(), (size_t)G * sizeof(float2), cudaMemcpyHostToDevice));
+        if (cfg->enable_3d) CREATE_TRY(cudaMalloc(&p->d_moment[0], (size_t)N * N * sizeof(float2)));
         p->fft_custom = true;
     } else if (4 * N <= 3 * G) {
         int n[1] = {G};
@@ -803,12 +809,12 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
         }
         // first transform pass out of place, sparse clear of the grid (and, after the last pass, of
         // the density map), second transform pass on the workspace
-        rc = transform_and_clear(p, sL, gridL, mapL, workL, uniform && last, false, nullptr, &launches);
+        rc = transform_and_clear(p, sL, gridL, mapL, workL, uniform && last, false, nullptr, L, &launches);
         if (rc) return rc;
         const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
         if (two_lanes && pass > 0) CU_TRY(p, cudaStreamWaitEvent(sL, p->ev_lane_comb[L ^ 1], 0));
-        launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, workL, p->d_ipsi, p->d_acc3,
-                            pass == 0 ? 1 : 0, sL);
+        launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->fft_custom ? p->d_moment[L] : workL,
+                            p->fft_custom ? 1 : 0, p->d_ipsi, p->d_acc3, pass == 0 ? 1 : 0, sL);
         ++launches;
         if (two_lanes) CU_TRY(p, cudaEventRecord(p->ev_lane_comb[L], sL));
     }
