@@ -222,24 +222,37 @@ __device__ __forceinline__ void load_powers(float2 *p, const float2 *row)
     p[2] = make_float2(hi.x, hi.y); p[3] = make_float2(hi.z, hi.w);
 }
 
-// stage A: G/16 radix-16 butterflies of stride G/16, twiddled by W_G^(k1 b)
-template <int LOG2G, int T>
-__device__ __forceinline__ void stage_a(float2 *s, int t, const float2 *tab)
+// stage A: G/16 radix-16 butterflies of stride G/16, twiddled by W_G^(k1 b).  `in(b, r)` supplies element
+// b + r G/16: from the sequence itself (SmemIn), or straight from global memory (consecutive threads,
+// consecutive b), which saves the pass that would first park the sequence in shared memory.
+struct SmemIn {
+    const float2 *s;
+    int l1p;
+    __device__ __forceinline__ float2 operator()(int b, int r) const { return s[pad16(b) + r * l1p]; }
+};
+
+// one butterfly of stage A: loads through `in`, results to at[r L1p]
+template <int LOG2G, class In>
+__device__ __forceinline__ void stage_a_butterfly(float2 *at, int b, const float2 *tab, const In &in)
+{
+    using P = Plan<LOG2G>;
+    float2 v[16], p[4];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) v[r] = in(b, r);
+    load_powers(p, tab + 4 * b);
+    dft16(v);
+    twiddle16(v, p);
+#pragma unroll
+    for (int r = 0; r < 16; ++r) at[r * P::L1p] = v[r];
+}
+
+template <int LOG2G, int T, class In>
+__device__ __forceinline__ void stage_a(float2 *s, int t, const float2 *tab, const In &in)
 {
     using P = Plan<LOG2G>;
     static_assert(P::L1 % T == 0, "threads per sequence must divide G / 16");
 #pragma unroll 1
-    for (int b = t; b < P::L1; b += T) {
-        float2 *at = s + pad16(b);
-        float2 v[16], p[4];
-#pragma unroll
-        for (int r = 0; r < 16; ++r) v[r] = at[r * P::L1p];
-        load_powers(p, tab + 4 * b);
-        dft16(v);
-        twiddle16(v, p);
-#pragma unroll
-        for (int r = 0; r < 16; ++r) at[r * P::L1p] = v[r];
-    }
+    for (int b = t; b < P::L1; b += T) stage_a_butterfly<LOG2G>(s + pad16(b), b, tab, in);
 }
 
 // stage B: inside block k1 (length L1), butterflies of radix R2 and stride S2, twiddled by W_L1^(k2 c)
@@ -323,15 +336,21 @@ __device__ __forceinline__ void stage_c(float2 *s, int t, const Out &out)
 // The whole transform of the sequence at `s` (element i at phys<LOG2G>(i)), by T threads, t = my index
 // among them.  Two CTA-wide barriers: every thread of the CTA must call it the same number of times;
 // the caller puts a barrier between its stores of the sequence and this call, and after it.
+// transform_from: stage A takes its inputs from `in` instead (the sequence need not be filled).
 // `tab`: fill_tables' output.  Stage C's results go to `out`.
-template <int LOG2G, int T, class Out>
-__device__ __forceinline__ void transform(float2 *s, int t, const float2 *tab, const Out &out)
+template <int LOG2G, int T, class In, class Out>
+__device__ __forceinline__ void transform_from(float2 *s, int t, const float2 *tab, const In &in, const Out &out)
 {
-    stage_a<LOG2G, T>(s, t, tab);
+    stage_a<LOG2G, T>(s, t, tab, in);
     __syncthreads();
     stage_b<LOG2G, T>(s, t, tab);
     __syncthreads();
     stage_c<LOG2G, T>(s, t, out);
+}
+template <int LOG2G, int T, class Out>
+__device__ __forceinline__ void transform(float2 *s, int t, const float2 *tab, const Out &out)
+{
+    transform_from<LOG2G, T>(s, t, tab, SmemIn{s, Plan<LOG2G>::L1p}, out);
 }
 
 }  // namespace fft

@@ -60,7 +60,6 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
     for (int y = blockIdx.x; y < G; y += gridDim.x) {
         const uint8_t *mrow = map + (size_t)(y / kTileH) * tiles_per_row(G);
         const float2 *src = grid + (size_t)y * G;
-        int any = 0;
         // the marks of this row's G / 128 tiles as bit masks (lane l looks at tiles l, l + 32, l + 64, l + 96)
         const int lane = t & 31;
         unsigned m[4];
@@ -68,29 +67,25 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
         for (int w = 0; w < 4; ++w)
             m[w] = 32 * w < kTiles ? __ballot_sync(0xffffffffu, lane + 32 * w < kTiles && __ldg(mrow + lane + 32 * w) != 0) : 0u;
         const unsigned long long marks_lo = ((unsigned long long)m[1] << 32) | m[0], marks_hi = ((unsigned long long)m[3] << 32) | m[2];
-        __syncthreads();                         // the previous row's last stage has read s_seq; the tables are filled
-#pragma unroll
-        for (int q = 0; q < G / T; ++q) {
-            const int x = t + q * T, tile = x / kTileW;
-            float2 v = make_float2(0.0f, 0.0f);
-            if (((tile < 64 ? marks_lo : marks_hi) >> (tile & 63)) & 1ull) {
-                v = __ldcs(src + x);             // read once: the clear zeroes it next
-                any = 1;
-            }
-            s_seq[fft::phys<LOG2G>(x)] = v;
-        }
-        any = __syncthreads_or(any);
         const ToWorkspace<LOG2G> to_work{work + (size_t)y * cols_block(LOG2G), half, N};
-        if (!any) {                              // an all-zero row transforms to zeros
+        if ((marks_lo | marks_hi) == 0ull) {     // an all-zero row transforms to zeros
             for (int n = t; n < half; n += T) {
                 to_work(n, nullptr, make_float2(0.0f, 0.0f));
                 to_work(G - half + n, nullptr, make_float2(0.0f, 0.0f));
             }
             continue;
         }
+        __syncthreads();                         // the previous row's last stage has read s_seq; the tables are filled
+        // stage A reads the row straight from the grid (consecutive threads, consecutive cells), through the tile marks
+        const auto from_grid = [&](int b, int r) {
+            const int x = b + r * P::L1, tile = x / kTileW;
+            float2 v = make_float2(0.0f, 0.0f);
+            if (((tile < 64 ? marks_lo : marks_hi) >> (tile & 63)) & 1ull) v = __ldcs(src + x);      // read once: the clear zeroes it next
+            return v;
+        };
         // the last stage hands its results straight to the workspace: only the needed columns, 8-byte
         // stores from consecutive threads to consecutive addresses
-        fft::transform<LOG2G, T>(s_seq, t, s_tab, to_work);
+        fft::transform_from<LOG2G, T>(s_seq, t, s_tab, from_grid, to_work);
     }
 }
 
@@ -108,10 +103,7 @@ k_fft_cols(const float2 *__restrict__ work, int N, const float2 *__restrict__ tw
     using P = fft::Plan<LOG2G>;
     constexpr int CB = cols_block(LOG2G);
     constexpr int G = 1 << LOG2G, NT = T * CT, SEQ = P::kPadded + kSkew;
-    constexpr int kW = C >= 2 ? 2 : 1;                   // float2 per load
-    constexpr int kLoads = (C * G / kW) / NT;            // loads per thread
-    constexpr int kBatch = kLoads < 16 ? kLoads : 16;
-    static_assert(CB % C == 0 && (C * G / kW) % NT == 0 && kLoads % kBatch == 0 && C % CT == 0, "a part must divide evenly among the threads");
+    static_assert(CB % C == 0 && (C * P::L1) % NT == 0 && C % CT == 0, "a part must divide evenly among the threads");
     extern __shared__ float2 s_dyn[];
     float2 *const s_tab = s_dyn, *const s_seq = s_dyn + P::kTabFloat2;       // [C][SEQ]
     const int tid = threadIdx.x, half = N >> 1;
@@ -125,33 +117,21 @@ k_fft_cols(const float2 *__restrict__ work, int N, const float2 *__restrict__ tw
         const int n0 = first < half ? first : G - half + (first - half);
         const float2 *src = work + (size_t)(first / CB) * ((size_t)G * CB) + first % CB;
         __syncthreads();                         // the previous pass has read s_seq; the tables are filled
-        // batches of loads, then their shared-memory stores
+        // stage A by all threads over (b, column), column fastest: its inputs come straight from the workspace,
+        // a warp reads 32 consecutive float2 when C = CB
 #pragma unroll 1
-        for (int u0 = 0; u0 < kLoads; u0 += kBatch) {
-            if constexpr (kW == 2) {
-                float4 ld[kBatch];
-#pragma unroll
-                for (int u = 0; u < kBatch; ++u) {
-                    const int idx = tid + (u0 + u) * NT, cp = idx % (C / 2), y = idx / (C / 2);
-                    ld[u] = __ldcs(reinterpret_cast<const float4 *>(src + (size_t)y * CB + 2 * cp));
-                }
-#pragma unroll
-                for (int u = 0; u < kBatch; ++u) {
-                    const int idx = tid + (u0 + u) * NT, cp = idx % (C / 2), y = idx / (C / 2);
-                    s_seq[(2 * cp) * SEQ + fft::phys<LOG2G>(y)] = make_float2(ld[u].x, ld[u].y);
-                    s_seq[(2 * cp + 1) * SEQ + fft::phys<LOG2G>(y)] = make_float2(ld[u].z, ld[u].w);
-                }
-            } else {
-                float2 ld[kBatch];
-#pragma unroll
-                for (int u = 0; u < kBatch; ++u) ld[u] = __ldcs(src + (size_t)(tid + (u0 + u) * NT) * CB);
-#pragma unroll
-                for (int u = 0; u < kBatch; ++u) s_seq[fft::phys<LOG2G>(tid + (u0 + u) * NT)] = ld[u];
-            }
+        for (int e = tid; e < C * P::L1; e += NT) {
+            const int c = e % C, b = e / C;
+            const float2 *col = src + c;
+            fft::stage_a_butterfly<LOG2G>(s_seq + c * SEQ + fft::pad16(b), b, s_tab,
+                                          [&](int bb, int r) { return __ldcs(col + (size_t)(bb + r * P::L1) * CB); });
         }
         __syncthreads();
 #pragma unroll 1
-        for (int c = grp; c < C; c += CT) fft::transform<LOG2G, T>(s_seq + c * SEQ, t, s_tab, fft::SmemOut{});
+        for (int c = grp; c < C; c += CT) fft::stage_b<LOG2G, T>(s_seq + c * SEQ, t, s_tab);
+        __syncthreads();
+#pragma unroll 1
+        for (int c = grp; c < C; c += CT) fft::stage_c<LOG2G, T>(s_seq + c * SEQ, t, fft::SmemOut{});
         __syncthreads();                         // output k of column c now sits at phys_out(k)
         if (IMAGE) {
             // step a7 fused: image[j][i] = Re F[m][n] (-1)^(n+m) / (psi(n) psi(m) omega Wsum), n = i - N/2, m = j - N/2
