@@ -8,8 +8,9 @@
 //
 //   k_r3_range      r3 range of the snapshot (Eq. 26) -- r3 = rho3 * s_c is monotone in s_c, so the
 //                   extremes sit at the band edges of the extreme baselines
-//   k_cheb_combine  correction + crop of one moment (complex: k_correct_crop keeps only Re) fused with
-//                   acc += exp(i 2 pi r3_p t3) c_k(alpha) M_pk per pixel, c_0 = J_0, c_k = 2 i^k J_k
+//   k_cheb_combine  correction + crop of one or two moments (complex: k_correct_crop keeps only Re) fused with
+//                   S_p += c_k(alpha) M_pk per pixel, c_0 = J_0, c_k = 2 i^k J_k, and after the slab's last
+//                   moment acc += exp(i 2 pi r3_p t3) S_p
 //   k_cheb_finish   image = Re(acc) / (omega Wsum); NaN outside the sphere constraint of Eq. 17
 #include <math_constants.h>
 
@@ -72,61 +73,77 @@ k_bessel_table(int K, double a_max, double *__restrict__ tab)
     tab[(size_t)k * (kJTab + 3) + m] = (x < 0.0 && (k & 1)) ? -v : v;
 }
 
-__device__ __forceinline__ double bessel_lookup(const double *__restrict__ row, double a_max, double inv_h, double x)
-{
-    double u = (x + a_max) * inv_h;                                 // 0 .. kJTab
-    u = fmin(fmax(u, 0.0), (double)kJTab);
-    int i = (int)u;
-    if (i > kJTab - 1) i = kJTab - 1;
-    const double f = u - (double)i;                                 // [0, 1]
-    const double *p = row + i;                                      // nodes i-1, i, i+1, i+2 (row is offset by one)
-    const double y0 = __ldg(p), y1 = __ldg(p + 1), y2 = __ldg(p + 2), y3 = __ldg(p + 3);
-    // 4-point Lagrange on nodes -1, 0, 1, 2
-    const double w0 = -f * (f - 1.0) * (f - 2.0) * (1.0 / 6.0);
-    const double w1 = (f + 1.0) * (f - 1.0) * (f - 2.0) * 0.5;
-    const double w2 = -(f + 1.0) * f * (f - 2.0) * 0.5;
-    const double w3 = (f + 1.0) * f * (f - 1.0) * (1.0 / 6.0);
-    return w0 * y0 + w1 * y1 + w2 * y2 + w3 * y3;
-}
-
+// One launch folds NM = 1 or 2 consecutive moments of a slab (orders k0, k0 + 1) into the slab's
+// sum S = sum_k i^k c_k(alpha) M_pk (per pixel: t3, the table position and the Lagrange weights are
+// computed once for both), and the slab's last launch adds exp(i 2 pi r3_p t3) S to the total -- the
+// phase is evaluated once per slab and pixel, not once per moment.
+//   first_k: k0 = 0 (S starts at zero);  last_k: k0 + NM = K (S goes into acc instead of back to memory);
+//   first_slab: acc starts at zero.
+template <int NM>
 __global__ void __launch_bounds__(256)
-k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, int k, double r3_p, double d_r3,
-               const double *__restrict__ jrow, double a_max, const float2 *__restrict__ F, int compact,
-               const double *__restrict__ ipsi, float2 *__restrict__ acc, int first)
+k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, int k0, double r3_p, double d_r3,
+               const double *__restrict__ jtab, double a_max, const float2 *__restrict__ F0, const float2 *__restrict__ F1,
+               int compact, const double *__restrict__ ipsi, float2 *__restrict__ slab, float2 *__restrict__ acc,
+               int first_k, int last_k, int first_slab)
 {
     const int i = blockIdx.x * 32 + (threadIdx.x & 31);
     const int j = blockIdx.y * 8 + (threadIdx.x >> 5);
     if (i >= N || j >= N) return;
     const size_t o = (size_t)j * N + i;
     const double t3 = t3_pixel(st->V, N, beta_rad, i, j);
-    float2 a = first ? make_float2(0.0f, 0.0f) : acc[o];
-    if (t3 == t3) {
-        const double two_pi = 6.283185307179586476925286766559;
-        const double alpha = two_pi * d_r3 * t3;                         // Eq. 20
-        double ck = a_max > 0.0 ? bessel_lookup(jrow, a_max, (double)kJTab / (2.0 * a_max), alpha)
-                                : (k == 0 ? 1.0 : 0.0);                  // Eq. 22 (alpha = 0 everywhere)
-        if (k > 0) ck *= 2.0;
-        double sp, cp;
-        sincospi(2.0 * r3_p * t3, &sp, &cp);
-        // w = exp(i 2 pi r3_p t3) * i^k * ck
-        double wr, wi;
-        switch (k & 3) {
-        case 0: wr = cp; wi = sp; break;
-        case 1: wr = -sp; wi = cp; break;
-        case 2: wr = -cp; wi = -sp; break;
-        default: wr = sp; wi = -cp; break;
-        }
-        // the moment at this pixel: the transform's unshifted output (compact: already cropped to [j][i]),
-        // (-1)^(n+m) of the centred grid, 1/(psi psi)
-        const int n = i - (N >> 1), m = j - (N >> 1);
-        const float2 f = __ldg(F + (compact ? o : (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n)));
-        double c = ipsi[i] * ipsi[j] * ck;
-        if ((n + m) & 1) c = -c;
-        wr *= c; wi *= c;
-        a.x += (float)(wr * f.x - wi * f.y);
-        a.y += (float)(wr * f.y + wi * f.x);
+    if (!(t3 == t3)) return;                                             // outside Eq. 17's sphere: k_cheb_finish writes NaN
+    const double two_pi = 6.283185307179586476925286766559;
+    float2 s = first_k ? make_float2(0.0f, 0.0f) : slab[o];
+    // the moments at this pixel: the transform's unshifted output (compact: already cropped to [j][i]),
+    // (-1)^(n+m) of the centred grid, 1/(psi psi)
+    const int n = i - (N >> 1), m = j - (N >> 1);
+    const size_t src = compact ? o : (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n);
+    double c = ipsi[i] * ipsi[j];
+    if ((n + m) & 1) c = -c;
+    // Eq. 20: alpha = 2 pi d t3; position in the Bessel table and 4-point Lagrange weights on nodes -1, 0, 1, 2
+    double w0 = 0.0, w1 = 0.0, w2 = 0.0, w3 = 0.0;
+    int node = 0;
+    if (a_max > 0.0) {
+        double u = (two_pi * d_r3 * t3 + a_max) * ((double)kJTab / (2.0 * a_max));      // 0 .. kJTab
+        u = fmin(fmax(u, 0.0), (double)kJTab);
+        node = (int)u;
+        if (node > kJTab - 1) node = kJTab - 1;
+        const double f = u - (double)node;                               // [0, 1]
+        w0 = -f * (f - 1.0) * (f - 2.0) * (1.0 / 6.0);
+        w1 = (f + 1.0) * (f - 1.0) * (f - 2.0) * 0.5;
+        w2 = -(f + 1.0) * f * (f - 2.0) * 0.5;
+        w3 = (f + 1.0) * f * (f - 1.0) * (1.0 / 6.0);
     }
-    acc[o] = a;
+#pragma unroll
+    for (int q = 0; q < NM; ++q) {
+        const int k = k0 + q;
+        double ck;                                                       // Eq. 22: c_0 = J_0, c_k = 2 J_k (times i^k below)
+        if (a_max > 0.0) {
+            const double *row = jtab + (size_t)k * (kJTab + 3) + node;   // nodes node-1 .. node+2 (rows are offset by one)
+            ck = w0 * __ldg(row) + w1 * __ldg(row + 1) + w2 * __ldg(row + 2) + w3 * __ldg(row + 3);
+        } else {
+            ck = k == 0 ? 1.0 : 0.0;                                     // alpha = 0 everywhere
+        }
+        if (k > 0) ck *= 2.0;
+        const float a = (float)(ck * c);
+        const float2 f = __ldg((q == 0 ? F0 : F1) + src);
+        switch (k & 3) {                                                 // s += i^k a f
+        case 0: s.x += a * f.x; s.y += a * f.y; break;
+        case 1: s.x -= a * f.y; s.y += a * f.x; break;
+        case 2: s.x -= a * f.x; s.y -= a * f.y; break;
+        default: s.x += a * f.y; s.y -= a * f.x; break;
+        }
+    }
+    if (!last_k) {
+        slab[o] = s;
+        return;
+    }
+    double sp, cp;
+    sincospi(2.0 * r3_p * t3, &sp, &cp);                                 // exp(i 2 pi r3_p t3)
+    float2 t = first_slab ? make_float2(0.0f, 0.0f) : acc[o];
+    t.x += (float)(cp * (double)s.x - sp * (double)s.y);
+    t.y += (float)(cp * (double)s.y + sp * (double)s.x);
+    acc[o] = t;
 }
 
 __global__ void __launch_bounds__(256)
@@ -163,13 +180,18 @@ void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream
     k_bessel_table<<<grid, 256, 0, stream>>>(K, a_max, d_tab);
 }
 
-void launch_cheb_combine(const Geometry &g, double beta_rad, const SnapState *st, int k, double r3_p, double d_r3,
-                         const double *d_tab, double a_max, const float2 *d_F, int compact, const double *d_ipsi,
-                         float2 *d_acc, int first, cudaStream_t stream)
+void launch_cheb_combine(const Geometry &g, double beta_rad, const SnapState *st, int k0, int n_moments, double r3_p,
+                         double d_r3, const double *d_tab, double a_max, const float2 *d_F0, const float2 *d_F1, int compact,
+                         const double *d_ipsi, float2 *d_slab, float2 *d_acc, int first_k, int last_k, int first_slab,
+                         cudaStream_t stream)
 {
     dim3 grid((g.N + 31) / 32, (g.N + 7) / 8);
-    k_cheb_combine<<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k, r3_p, d_r3, d_tab + (size_t)k * (kJTab + 3),
-                                             a_max, d_F, compact, d_ipsi, d_acc, first);
+    if (n_moments == 2)
+        k_cheb_combine<2><<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k0, r3_p, d_r3, d_tab, a_max, d_F0, d_F1, compact,
+                                                    d_ipsi, d_slab, d_acc, first_k, last_k, first_slab);
+    else
+        k_cheb_combine<1><<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k0, r3_p, d_r3, d_tab, a_max, d_F0, d_F0, compact,
+                                                    d_ipsi, d_slab, d_acc, first_k, last_k, first_slab);
 }
 
 void launch_cheb_finish(int N, double beta_rad, const SnapState *st, int apply_jacobian, const float2 *d_acc,

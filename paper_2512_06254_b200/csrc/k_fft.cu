@@ -95,7 +95,7 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
 // Sequences sit kSkew float2 apart beyond their padded length, so that the C columns of one grid row
 // fall on different banks when a row segment is stored.
 constexpr int kSkew = 4;
-template <int LOG2G, int C, int CT, int T, bool IMAGE>
+template <int LOG2G, int C, int CT, int T, int UA, bool IMAGE>
 __global__ void __launch_bounds__(T * CT)
 k_fft_cols(const float2 *__restrict__ work, int N, const float2 *__restrict__ tw, const double *__restrict__ ipsi,
            const SnapState *__restrict__ st, int apply_jacobian, float *__restrict__ image, float2 *__restrict__ moment)
@@ -119,7 +119,7 @@ k_fft_cols(const float2 *__restrict__ work, int N, const float2 *__restrict__ tw
         __syncthreads();                         // the previous pass has read s_seq; the tables are filled
         // stage A by all threads over (b, column), column fastest: its inputs come straight from the workspace,
         // a warp reads 32 consecutive float2 when C = CB
-#pragma unroll 1
+#pragma unroll UA
         for (int e = tid; e < C * P::L1; e += NT) {
             const int c = e % C, b = e / C;
             const float2 *col = src + c;
@@ -176,7 +176,7 @@ void rows_launch(const float2 *grid, float2 *work, const uint8_t *map, int N, co
     k_fft_rows<LOG2G, T, MINB><<<ctas, T, smem, stream>>>(grid, work, map, N, tw);
 }
 
-template <int LOG2G, int C, int CT, int T>
+template <int LOG2G, int C, int CT, int T, int UA>
 void cols_launch(const float2 *work, int N, const float2 *tw, const double *ipsi, const SnapState *st, int apply_jacobian,
                  float *image, float2 *moment, int n_sms, cudaStream_t stream)
 {
@@ -188,13 +188,13 @@ void cols_launch(const float2 *work, int N, const float2 *tw, const double *ipsi
     int ctas = per_sm * n_sms;
     if (ctas > N / C) ctas = N / C;
     if (image) {
-        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, UA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        k_fft_cols<LOG2G, C, CT, T, true><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image, moment);
+        k_fft_cols<LOG2G, C, CT, T, UA, true><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image, moment);
     } else {
-        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, UA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        k_fft_cols<LOG2G, C, CT, T, false><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image, moment);
+        k_fft_cols<LOG2G, C, CT, T, UA, false><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image, moment);
     }
 }
 
@@ -243,11 +243,11 @@ void launch_fft_cols(int N, int G, const float2 *d_work, const float2 *d_tw, con
                      int apply_jacobian, float *d_image, float2 *d_moment, int n_sms, cudaStream_t stream)
 {
     switch (log2_exact(G)) {
-    case 10: cols_launch<10, 8, 8, 64>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
-    case 11: cols_launch<11, 8, 4, 128>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
-    case 12: cols_launch<12, 4, 4, 128>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
-    case 13: cols_launch<13, 2, 2, 128>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
-    default: cols_launch<14, 1, 1, 512>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    case 10: cols_launch<10, 8, 8, 64, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    case 11: cols_launch<11, 8, 4, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    case 12: cols_launch<12, 4, 4, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    case 13: cols_launch<13, 2, 2, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    default: cols_launch<14, 1, 1, 512, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
     }
 }
 

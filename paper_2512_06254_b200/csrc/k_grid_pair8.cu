@@ -88,6 +88,16 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
         double rho1, rho2;
         rotate_baseline(st->V, in.uvw + 3 * j, rho1, rho2);
         const double rho3 = CHEB ? rotate_row3(st->V, in.uvw + 3 * j) : 0.0;
+        if (CHEB && tiles != nullptr && !count_rej && cheb.d > 0.0) {
+            // r3 = rho3 s_c is monotone along the task's channels (monotone channel scales: the plan passes
+            // `tiles` only then), and so is the slab index: a task whose end samples both fall on one side
+            // of slab cheb.p holds none of its samples.  (Not in the pass that counts the rejects.)
+            const double ra = __dmul_rn(rho3, __ldg(g.s + c_task));
+            const double rb = __dmul_rn(rho3, __ldg(g.s + min(c_task + kGroups * strip_len, g.n_c) - 1));
+            const int pa = min((int)floor((fmin(ra, rb) - cheb.r3_min) / (2.0 * cheb.d)), cheb.n_slab - 1);
+            const int pb = min((int)floor((fmax(ra, rb) - cheb.r3_min) / (2.0 * cheb.d)), cheb.n_slab - 1);
+            if (cheb.p < pa || cheb.p > pb) continue;
+        }
         const int c_lo = c_task + grp * strip_len + pre_k;        // my channel in batch 0
         const int c_hi = min(c_task + (grp + 1) * strip_len, g.n_c);
         const long long q_row = (long long)j * g.n_c;

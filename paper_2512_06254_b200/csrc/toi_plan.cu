@@ -80,7 +80,7 @@ struct toi_plan {
 
     // near-coplanar (3-D) mode (cfg.enable_3d): complex accumulator, r3 range on the device and in
     // pinned host memory, Bessel table; the passes run on d_grid / d_work like the 2-D path
-    float2 *d_acc3 = nullptr;
+    float2 *d_acc3 = nullptr, *d_slab3 = nullptr;        // total and per-slab sums of the 3-D mode, [N][N] each
     double *d_r3 = nullptr, *h_r3 = nullptr, *d_jtab = nullptr;
     // second lane of the 3-D mode (hand-written transform only): odd passes grid, transform and combine
     // on their own grid / workspace / tile map on s_lane1, so that one pass's transform runs under the
@@ -88,7 +88,7 @@ struct toi_plan {
     float2 *d_grid1 = nullptr, *d_grid1_alloc = nullptr, *d_work1 = nullptr;
     uint8_t *d_tiles1 = nullptr;
     cudaStream_t s_lane1 = nullptr;
-    cudaEvent_t ev_lane_grid[2] = {}, ev_lane_comb[2] = {}, ev_lane_setup = nullptr;
+    cudaEvent_t ev_lane_grid[2] = {}, ev_lane_comb[2] = {}, ev_lane_setup = nullptr, ev_lane_cols0 = nullptr;
     double s_min = 0, s_max = 0;
     cudaEvent_t ev3_a = nullptr, ev3_b = nullptr;
 
@@ -205,7 +205,7 @@ int free_plan(toi_plan *p)
     }
     if (p->ev_tail) cudaEventDestroy(p->ev_tail);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
-    cudaFree(p->d_acc3); cudaFree(p->d_r3); cudaFree(p->d_jtab);
+    cudaFree(p->d_acc3); cudaFree(p->d_slab3); cudaFree(p->d_r3); cudaFree(p->d_jtab);
     if (p->s_lane1) cudaStreamSynchronize(p->s_lane1);
     cudaFree(p->d_grid1_alloc); cudaFree(p->d_work1); cudaFree(p->d_tiles1);
     for (int k = 0; k < 2; ++k) {
@@ -213,6 +213,7 @@ int free_plan(toi_plan *p)
         if (p->ev_lane_comb[k]) cudaEventDestroy(p->ev_lane_comb[k]);
     }
     if (p->ev_lane_setup) cudaEventDestroy(p->ev_lane_setup);
+    if (p->ev_lane_cols0) cudaEventDestroy(p->ev_lane_cols0);
     if (p->s_lane1) cudaStreamDestroy(p->s_lane1);
     cudaFreeHost(p->h_r3);
     if (p->ev3_a) cudaEventDestroy(p->ev3_a);
@@ -252,7 +253,7 @@ uint8_t *gridder_tile_map(toi_plan *p, cudaStream_t stream, bool sliding, uint8_
 // complex transform is left in the workspace (cuFFT) or, cropped, in d_moment[lane] (hand-written
 // transform).  `timed`: record the stage events of the 2-D path.
 int transform_and_clear(toi_plan *p, cudaStream_t stream, float2 *d_grid, uint8_t *d_tiles, float2 *d_work,
-                        bool clear_density, bool timed, float *d_image, int lane, int *launches)
+                        bool clear_density, bool timed, float *d_image, int lane, cudaEvent_t before_cols, int *launches)
 {
     const Geometry &g = p->geo;
     cufftComplex *A = (cufftComplex *)d_grid, *F = (cufftComplex *)d_work;
@@ -270,6 +271,7 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, float2 *d_grid, uint8_
     launch_clear_tiles(d_grid, clear_density ? p->d_dens : nullptr, g.G, d_tiles, stream);
     ++*launches;
     if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
+    if (before_cols) CU_TRY(p, cudaStreamWaitEvent(stream, before_cols, 0));     // what still reads this lane's moment
     if (p->fft_custom) {
         launch_fft_cols(g.N, g.G, d_work, p->d_tw, p->d_ipsi, p->d_state, p->apply_jacobian, d_image,
                         d_image ? nullptr : p->d_moment[lane], p->n_sms, stream);
@@ -333,7 +335,7 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     // pass when the hand-written transform runs: ms_crop is then ~0 and ms_fft holds both)
     float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
     ++p->ring_pos;
-    rc = transform_and_clear(p, stream, p->d_grid, p->d_tiles_grid, p->d_work, uniform, true, img, 0, &launches);
+    rc = transform_and_clear(p, stream, p->d_grid, p->d_tiles_grid, p->d_work, uniform, true, img, 0, nullptr, &launches);
     if (rc) return rc;
     CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
     CU_TRY(p, cudaEventRecord(p->ev_done, stream));
@@ -534,6 +536,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     }
     if (cfg->enable_3d) {
         CREATE_TRY(cudaMalloc(&p->d_acc3, (size_t)N * N * sizeof(float2)));
+        CREATE_TRY(cudaMalloc(&p->d_slab3, (size_t)N * N * sizeof(float2)));
         CREATE_TRY(cudaMalloc(&p->d_r3, 2 * sizeof(double)));
         CREATE_TRY(cudaMalloc(&p->d_jtab, bessel_table_doubles(64) * sizeof(double)));
         CREATE_TRY(cudaMallocHost(&p->h_r3, 2 * sizeof(double)));
@@ -553,6 +556,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
                 CREATE_TRY(cudaEventCreateWithFlags(&p->ev_lane_comb[k], cudaEventDisableTiming));
             }
             CREATE_TRY(cudaEventCreateWithFlags(&p->ev_lane_setup, cudaEventDisableTiming));
+            CREATE_TRY(cudaEventCreateWithFlags(&p->ev_lane_cols0, cudaEventDisableTiming));
         }
     }
     CREATE_TRY(cudaMalloc(&p->d_images, (size_t)p->ring_depth * N * N * sizeof(float)));
@@ -776,20 +780,23 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     const double a_max = d > 0.0 ? 2.0 * 3.14159265358979323846 * d * t3_max * (1.0 + 1e-9) : 0.0;
     launch_bessel_table(K, a_max, p->d_jtab, stream);
     ++launches;
-    // Two lanes (when the second set of buffers exists): even passes on `stream`, odd passes on s_lane1,
-    // each on its own grid / tile map / workspace.  A pass's transform (shared-memory and DRAM bound)
-    // then runs under the next pass's gridding (issue bound).  What the passes share is kept in order by
-    // events: the task counter and the density map (gridder p + 1 waits for gridder p), the accumulator
-    // (combination p + 1 waits for combination p).
+    // Two lanes (when the second set of buffers exists): even orders k on `stream`, odd ones on s_lane1,
+    // each on its own grid / tile map / workspace / moment.  What the passes share is kept in order by
+    // events: the task counter and the density map (gridder p + 1 waits for gridder p), the slab and total
+    // sums (a combination waits for the one before), a lane's moment (its next column pass waits for the
+    // combination that read it).  The two moments of a pair (k even, k + 1) are folded in by ONE
+    // combination launch on the odd lane; a slab's unpaired last order (K odd), and every order when
+    // there is one lane, by a launch of its own.
     const bool two_lanes = p->d_grid1 != nullptr;
     if (two_lanes) {
         CU_TRY(p, cudaEventRecord(p->ev_lane_setup, stream));
         CU_TRY(p, cudaStreamWaitEvent(p->s_lane1, p->ev_lane_setup, 0));
     }
     const int n_passes = slabs_run * K;
+    bool have_comb[2] = {false, false};
     for (int pass = 0; pass < n_passes; ++pass) {
         const int sp = pass / K, k = pass % K;
-        const int L = two_lanes ? (pass & 1) : 0;
+        const int L = two_lanes ? (k & 1) : 0;
         cudaStream_t sL = L ? p->s_lane1 : stream;
         float2 *gridL = L ? p->d_grid1 : p->d_grid, *workL = L ? p->d_work1 : p->d_work;
         uint8_t *mapL = L ? p->d_tiles1 : p->d_tiles_grid;
@@ -809,17 +816,28 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
         }
         // first transform pass out of place, sparse clear of the grid (and, after the last pass, of
         // the density map), second transform pass on the workspace
-        rc = transform_and_clear(p, sL, gridL, mapL, workL, uniform && last, false, nullptr, L, &launches);
+        rc = transform_and_clear(p, sL, gridL, mapL, workL, uniform && last, false, nullptr, L,
+                                 two_lanes && have_comb[L ^ 1] ? p->ev_lane_comb[L ^ 1] : nullptr, &launches);
         if (rc) return rc;
+        if (two_lanes && L == 0 && k != K - 1) {         // the odd lane's combination takes this moment along
+            CU_TRY(p, cudaEventRecord(p->ev_lane_cols0, sL));
+            continue;
+        }
+        const int nm = two_lanes && L == 1 ? 2 : 1, k0 = k - (nm - 1);
         const double r3_p = d > 0.0 ? r3_min + (2.0 * sp + 1.0) * d : r3_min;
-        if (two_lanes && pass > 0) CU_TRY(p, cudaStreamWaitEvent(sL, p->ev_lane_comb[L ^ 1], 0));
-        launch_cheb_combine(g, beta, p->d_state, k, r3_p, d, p->d_jtab, a_max, p->fft_custom ? p->d_moment[L] : workL,
-                            p->fft_custom ? 1 : 0, p->d_ipsi, p->d_acc3, pass == 0 ? 1 : 0, sL);
+        if (nm == 2) CU_TRY(p, cudaStreamWaitEvent(sL, p->ev_lane_cols0, 0));
+        if (two_lanes && have_comb[L ^ 1]) CU_TRY(p, cudaStreamWaitEvent(sL, p->ev_lane_comb[L ^ 1], 0));
+        const float2 *F0 = p->fft_custom ? p->d_moment[nm == 2 ? 0 : L] : workL;
+        launch_cheb_combine(g, beta, p->d_state, k0, nm, r3_p, d, p->d_jtab, a_max, F0, p->d_moment[1], p->fft_custom ? 1 : 0,
+                            p->d_ipsi, p->d_slab3, p->d_acc3, k0 == 0 ? 1 : 0, k0 + nm == K ? 1 : 0, sp == 0 ? 1 : 0, sL);
         ++launches;
-        if (two_lanes) CU_TRY(p, cudaEventRecord(p->ev_lane_comb[L], sL));
+        if (two_lanes) {
+            CU_TRY(p, cudaEventRecord(p->ev_lane_comb[L], sL));
+            have_comb[L] = true;
+        }
     }
     // the last combination may sit on the other lane
-    if (two_lanes && n_passes > 0 && ((n_passes - 1) & 1)) CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_lane_comb[1], 0));
+    if (two_lanes && have_comb[1]) CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_lane_comb[1], 0));
     launch_cheb_finish(g.N, beta, p->d_state, p->apply_jacobian, p->d_acc3, img, stream);
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev3_b, stream));
