@@ -281,6 +281,25 @@ def test_edge_non_default_grid_size():
     _assert_image(img, img_o, "G=384")
 
 
+@pytest.mark.parametrize("N,G", [(528, 1024), (1536, 2048), (752, 2048), (1040, 4096)])
+def test_hand_written_transform_with_other_crops(N, G):
+    """k_fft_rows / k_fft_cols take G = 2^10 .. 2^14 with G >= 4N/3 and N a multiple of 16; every other
+    test runs them at G = 2N.  Here the crop keeps a non-power-of-two N (the two bands of needed columns
+    [0, N/2) and [G - N/2, G) and the blocks of the workspace between the passes end on odd multiples
+    of the block width), up to the limit N = 3G/4.  Image against the oracle's, natural and uniform."""
+    wl = _reduced2(n_ant=12, n_chan=96, image_size=N)
+    snap = snapshot_np(wl)
+    for weighting in ("natural", "uniform"):
+        rc, img_o, info_o, _ = _oracle(snap, N, wl.cell_size_deg, weighting, G=G, pol_a=0, pol_b=3)
+        assert rc == 0 and info_o["n_gridded"] > 0
+        with GpuImager(snap, N, wl.cell_size_deg, weighting, grid_size=G, pol_a=0, pol_b=3) as gi:
+            img, info, _ = gi.image()
+            img2, _, _ = gi.image()                  # the workspace and the tile map are reused
+        assert info["n_gridded"] == info_o["n_gridded"]
+        _assert_image(img, img_o, f"N={N} G={G} {weighting}")
+        _assert_image(img2, img_o, f"N={N} G={G} {weighting} (second call)")
+
+
 @pytest.mark.parametrize("gridder", ALL_GRIDDERS)
 @pytest.mark.parametrize("G", [198, 202, 136])
 def test_edge_grid_half_size_odd_or_tight(G, gridder):
