@@ -54,14 +54,15 @@ __device__ __forceinline__ double t3_pixel(const double *V, int N, double beta_r
 }
 
 // J_k on a uniform grid of n_tab + 1 points over [-a_max, a_max] (one extra node on each side for
-// the 4-point stencil), by the CUDA math library's jn: K x (n_tab + 3) doubles, once per snapshot.
-// The combination kernel interpolates it (4-point Lagrange: error <= (3/128) h^4 max|d4 J_k| ~ 1e-11
-// for h = 2 a_max / 4096, a_max <= ~10) instead of calling jn per pixel and pass, which costs
+// the 4-point stencil), by the CUDA math library's jn in fp64, stored as K x (n_tab + 3) floats, once per snapshot.
+// The combination kernel interpolates it (4-point Lagrange: truncation <= (3/128) h^4 max|d4 J_k| ~ 1e-11
+// for h = 2 a_max / 4096, a_max <= ~10; the fp32 table and weights add ~1e-7, against an expansion error
+// of 1e-4 .. 1e-2 by Eq. 25) instead of calling jn per pixel and pass, which costs
 // several hundred fp64 instructions (a per-pixel Miller recurrence was slower still).
 constexpr int kJTab = 4096;
 
 __global__ void __launch_bounds__(256)
-k_bessel_table(int K, double a_max, double *__restrict__ tab)
+k_bessel_table(int K, double a_max, float *__restrict__ tab)
 {
     const int m = blockIdx.x * blockDim.x + threadIdx.x;           // 0 .. kJTab + 2
     const int k = blockIdx.y;
@@ -70,7 +71,7 @@ k_bessel_table(int K, double a_max, double *__restrict__ tab)
     const double x = -a_max + (double)(m - 1) * h;
     // J_k(-x) = (-1)^k J_k(x); the centre node is x = 0 exactly, where jn(k > 1, 0) returns NaN
     const double v = fabs(x) < 1e-300 ? (k == 0 ? 1.0 : 0.0) : jn(k, fabs(x));
-    tab[(size_t)k * (kJTab + 3) + m] = (x < 0.0 && (k & 1)) ? -v : v;
+    tab[(size_t)k * (kJTab + 3) + m] = (float)((x < 0.0 && (k & 1)) ? -v : v);
 }
 
 // One launch folds NM = 1 or 2 consecutive moments of a slab (orders k0, k0 + 1) into the slab's
@@ -82,7 +83,7 @@ k_bessel_table(int K, double a_max, double *__restrict__ tab)
 template <int NM>
 __global__ void __launch_bounds__(256)
 k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, int k0, double r3_p, double d_r3,
-               const double *__restrict__ jtab, double a_max, const float2 *__restrict__ F0, const float2 *__restrict__ F1,
+               const float *__restrict__ jtab, double a_max, double inv_h, const float2 *__restrict__ F0, const float2 *__restrict__ F1,
                int compact, const double *__restrict__ ipsi, float2 *__restrict__ slab, float2 *__restrict__ acc,
                int first_k, int last_k, int first_slab)
 {
@@ -100,32 +101,34 @@ k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, 
     const size_t src = compact ? o : (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n);
     double c = ipsi[i] * ipsi[j];
     if ((n + m) & 1) c = -c;
-    // Eq. 20: alpha = 2 pi d t3; position in the Bessel table and 4-point Lagrange weights on nodes -1, 0, 1, 2
-    double w0 = 0.0, w1 = 0.0, w2 = 0.0, w3 = 0.0;
+    // Eq. 20: alpha = 2 pi d t3; position in the Bessel table in fp64, the 4-point Lagrange weights on nodes
+    // -1, 0, 1, 2 and the interpolation in fp32 (|J_k| <= 1: 1e-7 absolute)
+    float w0 = 0.0f, w1 = 0.0f, w2 = 0.0f, w3 = 0.0f;
     int node = 0;
     if (a_max > 0.0) {
-        double u = (two_pi * d_r3 * t3 + a_max) * ((double)kJTab / (2.0 * a_max));      // 0 .. kJTab
+        double u = (two_pi * d_r3 * t3 + a_max) * inv_h;                 // 0 .. kJTab
         u = fmin(fmax(u, 0.0), (double)kJTab);
         node = (int)u;
         if (node > kJTab - 1) node = kJTab - 1;
-        const double f = u - (double)node;                               // [0, 1]
-        w0 = -f * (f - 1.0) * (f - 2.0) * (1.0 / 6.0);
-        w1 = (f + 1.0) * (f - 1.0) * (f - 2.0) * 0.5;
-        w2 = -(f + 1.0) * f * (f - 2.0) * 0.5;
-        w3 = (f + 1.0) * f * (f - 1.0) * (1.0 / 6.0);
+        const float f = (float)(u - (double)node);                       // [0, 1]
+        w0 = -f * (f - 1.0f) * (f - 2.0f) * (1.0f / 6.0f);
+        w1 = (f + 1.0f) * (f - 1.0f) * (f - 2.0f) * 0.5f;
+        w2 = -(f + 1.0f) * f * (f - 2.0f) * 0.5f;
+        w3 = (f + 1.0f) * f * (f - 1.0f) * (1.0f / 6.0f);
     }
+    const float cf = (float)c;
 #pragma unroll
     for (int q = 0; q < NM; ++q) {
         const int k = k0 + q;
-        double ck;                                                       // Eq. 22: c_0 = J_0, c_k = 2 J_k (times i^k below)
+        float ck;                                                        // Eq. 22: c_0 = J_0, c_k = 2 J_k (times i^k below)
         if (a_max > 0.0) {
-            const double *row = jtab + (size_t)k * (kJTab + 3) + node;   // nodes node-1 .. node+2 (rows are offset by one)
+            const float *row = jtab + (size_t)k * (kJTab + 3) + node;    // nodes node-1 .. node+2 (rows are offset by one)
             ck = w0 * __ldg(row) + w1 * __ldg(row + 1) + w2 * __ldg(row + 2) + w3 * __ldg(row + 3);
         } else {
-            ck = k == 0 ? 1.0 : 0.0;                                     // alpha = 0 everywhere
+            ck = k == 0 ? 1.0f : 0.0f;                                   // alpha = 0 everywhere
         }
-        if (k > 0) ck *= 2.0;
-        const float a = (float)(ck * c);
+        if (k > 0) ck *= 2.0f;
+        const float a = ck * cf;
         const float2 f = __ldg((q == 0 ? F0 : F1) + src);
         switch (k & 3) {                                                 // s += i^k a f
         case 0: s.x += a * f.x; s.y += a * f.y; break;
@@ -171,9 +174,9 @@ void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s
     k_r3_range<<<1, 256, 0, stream>>>(n_b, d_uvw, st, s_min, s_max, d_out);
 }
 
-size_t bessel_table_doubles(int K) { return (size_t)K * (kJTab + 3); }
+size_t bessel_table_floats(int K) { return (size_t)K * (kJTab + 3); }
 
-void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream)
+void launch_bessel_table(int K, double a_max, float *d_tab, cudaStream_t stream)
 {
     if (!(a_max > 0.0)) return;
     dim3 grid((kJTab + 3 + 255) / 256, K);
@@ -181,16 +184,17 @@ void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream
 }
 
 void launch_cheb_combine(const Geometry &g, double beta_rad, const SnapState *st, int k0, int n_moments, double r3_p,
-                         double d_r3, const double *d_tab, double a_max, const float2 *d_F0, const float2 *d_F1, int compact,
+                         double d_r3, const float *d_tab, double a_max, const float2 *d_F0, const float2 *d_F1, int compact,
                          const double *d_ipsi, float2 *d_slab, float2 *d_acc, int first_k, int last_k, int first_slab,
                          cudaStream_t stream)
 {
     dim3 grid((g.N + 31) / 32, (g.N + 7) / 8);
+    const double inv_h = a_max > 0.0 ? (double)kJTab / (2.0 * a_max) : 0.0;
     if (n_moments == 2)
-        k_cheb_combine<2><<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k0, r3_p, d_r3, d_tab, a_max, d_F0, d_F1, compact,
+        k_cheb_combine<2><<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k0, r3_p, d_r3, d_tab, a_max, inv_h, d_F0, d_F1, compact,
                                                     d_ipsi, d_slab, d_acc, first_k, last_k, first_slab);
     else
-        k_cheb_combine<1><<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k0, r3_p, d_r3, d_tab, a_max, d_F0, d_F0, compact,
+        k_cheb_combine<1><<<grid, 256, 0, stream>>>(g.N, g.G, beta_rad, st, k0, r3_p, d_r3, d_tab, a_max, inv_h, d_F0, d_F0, compact,
                                                     d_ipsi, d_slab, d_acc, first_k, last_k, first_slab);
 }
 

@@ -268,10 +268,10 @@ void launch_fft_cols(int N, int G, const float2 *d_work, const float2 *d_tw, con
                      int apply_jacobian, float *d_image, float2 *d_moment, int n_sms, cudaStream_t stream);
 void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s_min, double s_max, double *d_out,
                      cudaStream_t stream);
-size_t bessel_table_doubles(int K);
-void launch_bessel_table(int K, double a_max, double *d_tab, cudaStream_t stream);
+size_t bessel_table_floats(int K);
+void launch_bessel_table(int K, double a_max, float *d_tab, cudaStream_t stream);
 void launch_cheb_combine(const Geometry &g, double beta_rad, const SnapState *st, int k0, int n_moments, double r3_p,
-                         double d_r3, const double *d_tab, double a_max, const float2 *d_F0, const float2 *d_F1, int compact,
+                         double d_r3, const float *d_tab, double a_max, const float2 *d_F0, const float2 *d_F1, int compact,
                          const double *d_ipsi, float2 *d_slab, float2 *d_acc, int first_k, int last_k, int first_slab,
                          cudaStream_t stream);
 void launch_cheb_finish(int N, double beta_rad, const SnapState *st, int apply_jacobian, const float2 *d_acc,

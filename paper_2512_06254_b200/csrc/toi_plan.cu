@@ -81,7 +81,8 @@ struct toi_plan {
     // near-coplanar (3-D) mode (cfg.enable_3d): complex accumulator, r3 range on the device and in
     // pinned host memory, Bessel table; the passes run on d_grid / d_work like the 2-D path
     float2 *d_acc3 = nullptr, *d_slab3 = nullptr;        // total and per-slab sums of the 3-D mode, [N][N] each
-    double *d_r3 = nullptr, *h_r3 = nullptr, *d_jtab = nullptr;
+    double *d_r3 = nullptr, *h_r3 = nullptr;
+    float *d_jtab = nullptr;                             // Bessel table of the 3-D mode
     // second lane of the 3-D mode (hand-written transform only): odd passes grid, transform and combine
     // on their own grid / workspace / tile map on s_lane1, so that one pass's transform runs under the
     // next pass's gridding; the gridders and the combinations of the two lanes are chained by events
@@ -538,7 +539,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
         CREATE_TRY(cudaMalloc(&p->d_acc3, (size_t)N * N * sizeof(float2)));
         CREATE_TRY(cudaMalloc(&p->d_slab3, (size_t)N * N * sizeof(float2)));
         CREATE_TRY(cudaMalloc(&p->d_r3, 2 * sizeof(double)));
-        CREATE_TRY(cudaMalloc(&p->d_jtab, bessel_table_doubles(64) * sizeof(double)));
+        CREATE_TRY(cudaMalloc(&p->d_jtab, bessel_table_floats(64) * sizeof(float)));
         CREATE_TRY(cudaMallocHost(&p->h_r3, 2 * sizeof(double)));
         CREATE_TRY(cudaEventCreate(&p->ev3_a));
         CREATE_TRY(cudaEventCreate(&p->ev3_b));
