@@ -5,16 +5,17 @@
 // Only the N columns n and N rows m the crop keeps are ever needed, and only 2-3 % of the grid is
 // non-zero.  Two kernels, both built on the shared-memory FFT of fft_smem.cuh:
 //   k_fft_rows   one CTA per grid row: the row is read THROUGH THE TILE MAP of the sparse clear (tiles
-//                the gridder did not mark are known to be zero and are not read: 25 MB instead of
-//                134 MB at config 2), transformed along x, and only the N needed columns are written
-//                to the workspace (a row without a marked tile writes zeros and skips the transform);
-//   k_fft_cols   one CTA per C adjacent needed columns: read strided (C x 8 B per row), transformed
+//                the gridder did not mark are known to be zero and are not read: 36 MB instead of
+//                134 MB at config 2) straight into the first stage's registers, transformed along x,
+//                and only the N needed columns are written to the workspace, in blocks of 4 columns
+//                (a row without a marked tile writes zeros and skips the transform);
+//   k_fft_cols   one CTA per block of needed columns: read as one contiguous run, transformed
 //                along y, and only the N needed rows leave the SM -- either as the finished image
 //                pixel Re F (-1)^(n+m) / (psi psi omega Wsum) (correction, crop and normalisation of
 //                step a7 fused: the transformed grid is never written back), or, for the Chebyshev
-//                moments of the 3-D mode, as complex values in place.
+//                moments of the 3-D mode, as the cropped complex moment [N][N].
 // cuFFT needs G x G reads and writes in both passes, a separate crop kernel, and cannot skip zeros.
-// For G = 2^10 .. 2^13 with G >= 4N/3 and N a multiple of 16; other shapes stay on cuFFT.
+// For G = 2^10 .. 2^14 with G >= 4N/3 and N a multiple of 16; other shapes stay on cuFFT.
 #include "fft_smem.cuh"
 #include "toi_internal.cuh"
 
