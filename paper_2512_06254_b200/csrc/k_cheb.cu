@@ -91,16 +91,21 @@ k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, 
     const int j = blockIdx.y * 8 + (threadIdx.x >> 5);
     if (i >= N || j >= N) return;
     const size_t o = (size_t)j * N + i;
+    // the moments at this pixel: the transform's unshifted output (compact: already cropped to [j][i]),
+    // (-1)^(n+m) of the centred grid, 1/(psi psi).  Everything that does not depend on t3 is requested
+    // first, so that its latency runs under the fp64 work below.
+    const int n = i - (N >> 1), m = j - (N >> 1);
+    const size_t src = compact ? o : (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n);
+    float2 fm[NM];
+    fm[0] = __ldcs(F0 + src);
+    if (NM == 2) fm[NM - 1] = __ldcs(F1 + src);
+    float2 s = make_float2(0.0f, 0.0f);
+    if (!first_k) s = __ldcs(slab + o);
+    double c = ipsi[i] * ipsi[j];
+    if ((n + m) & 1) c = -c;
     const double t3 = t3_pixel(st->V, N, beta_rad, i, j);
     if (!(t3 == t3)) return;                                             // outside Eq. 17's sphere: k_cheb_finish writes NaN
     const double two_pi = 6.283185307179586476925286766559;
-    float2 s = first_k ? make_float2(0.0f, 0.0f) : slab[o];
-    // the moments at this pixel: the transform's unshifted output (compact: already cropped to [j][i]),
-    // (-1)^(n+m) of the centred grid, 1/(psi psi)
-    const int n = i - (N >> 1), m = j - (N >> 1);
-    const size_t src = compact ? o : (size_t)(m < 0 ? m + G : m) * G + (n < 0 ? n + G : n);
-    double c = ipsi[i] * ipsi[j];
-    if ((n + m) & 1) c = -c;
     // Eq. 20: alpha = 2 pi d t3; position in the Bessel table in fp64, the 4-point Lagrange weights on nodes
     // -1, 0, 1, 2 and the interpolation in fp32 (|J_k| <= 1: 1e-7 absolute)
     float w0 = 0.0f, w1 = 0.0f, w2 = 0.0f, w3 = 0.0f;
@@ -129,7 +134,7 @@ k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, 
         }
         if (k > 0) ck *= 2.0f;
         const float a = ck * cf;
-        const float2 f = __ldg((q == 0 ? F0 : F1) + src);
+        const float2 f = fm[q];
         switch (k & 3) {                                                 // s += i^k a f
         case 0: s.x += a * f.x; s.y += a * f.y; break;
         case 1: s.x -= a * f.y; s.y += a * f.x; break;
@@ -138,7 +143,7 @@ k_cheb_combine(int N, int G, double beta_rad, const SnapState *__restrict__ st, 
         }
     }
     if (!last_k) {
-        slab[o] = s;
+        __stcs(slab + o, s);
         return;
     }
     double sp, cp;
