@@ -296,7 +296,9 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, float2 *d_grid, uint8_
 }
 
 // Enqueue stages a1..a7 for the snapshot resident at `in` on `stream`; returns the image slot.
-int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **d_image_out)
+// `timed`: record the per-stage events toi_snapshot_info is read from (a timed event between two kernels
+// costs 1-2 us of the stream's time; only calls that ask for the info pay for them).
+int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **d_image_out, bool timed)
 {
     const Geometry &g = p->geo;
     const size_t GG = (size_t)g.G * g.G;
@@ -309,7 +311,7 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     // a1-a2: plane fit (also resets the per-snapshot accumulators)
     launch_planefit(g, in.uvw, p->S1, p->S2, p->inject ? p->d_V_inject : nullptr, p->d_state, stream);
     ++launches;
-    CU_TRY(p, cudaEventRecord(p->ev[EV_FIT], stream));
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_FIT], stream));
     // a4: uniform-weighting density pass
     const float *dens = nullptr;
     if (uniform) {
@@ -317,7 +319,7 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
         dens = p->d_dens;
         ++launches;
     }
-    CU_TRY(p, cudaEventRecord(p->ev[EV_WEIGHT], stream));
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_WEIGHT], stream));
     // a3 + a5: cell indices and gridding onto the zero grid
     const bool sliding = p->cfg.gridder != TOI_GRIDDER_ATOMIC;
     uint8_t *tiles = gridder_tile_map(p, stream, sliding, p->d_tiles_grid);
@@ -326,7 +328,7 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     else
         launch_grid_atomic(g, in, p->d_state, dens, p->d_grid, stream);
     launches += tiles ? 1 : 2;
-    CU_TRY(p, cudaEventRecord(p->ev[EV_GRID], stream));
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_GRID], stream));
     if (p->keep_grid) {
         CU_TRY(p, cudaMemcpyAsync(p->d_grid_keep, p->d_grid, GG * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
         if (uniform) CU_TRY(p, cudaMemcpyAsync(p->d_dens_keep, p->d_dens, GG * sizeof(float), cudaMemcpyDeviceToDevice, stream));
@@ -336,9 +338,9 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     // pass when the hand-written transform runs: ms_crop is then ~0 and ms_fft holds both)
     float *img = p->d_images + (size_t)(p->ring_pos % p->ring_depth) * g.N * g.N;
     ++p->ring_pos;
-    rc = transform_and_clear(p, stream, p->d_grid, p->d_tiles_grid, p->d_work, uniform, true, img, 0, nullptr, &launches);
+    rc = transform_and_clear(p, stream, p->d_grid, p->d_tiles_grid, p->d_work, uniform, timed, img, 0, nullptr, &launches);
     if (rc) return rc;
-    CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
     CU_TRY(p, cudaEventRecord(p->ev_done, stream));
     CU_TRY(p, cudaGetLastError());
     p->last_in = in;
@@ -619,7 +621,8 @@ int toi_image_snapshot(toi_plan *p, const double *uvw_m, const void *vis, const 
     CU_TRY(p, cudaSetDevice(p->cfg.device));
     cudaStream_t stream = cuda_stream ? (cudaStream_t)cuda_stream : p->s_compute;
     Inputs in;
-    CU_TRY(p, cudaEventRecord(p->ev[EV_START], stream));
+    const bool timed = info != nullptr;
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_START], stream));
     const bool host = p->cfg.input_location == TOI_MEM_HOST;
     if (host) {
         p->snap_slot ^= 1;
@@ -628,8 +631,8 @@ int toi_image_snapshot(toi_plan *p, const double *uvw_m, const void *vis, const 
     } else {
         in.uvw = uvw_m; in.vis = (const float2 *)vis; in.weights = weights; in.flags = flags;
     }
-    CU_TRY(p, cudaEventRecord(p->ev[EV_H2D], stream));
-    int rc = enqueue_imaging(p, in, stream, d_image_out);
+    if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_H2D], stream));
+    int rc = enqueue_imaging(p, in, stream, d_image_out, timed);
     if (rc) return rc;
     if (info) return read_info(p, stream, info, host);
     return TOI_OK;
@@ -1003,10 +1006,12 @@ int toi_image_stream(toi_plan *p, int64_t n_snapshots, toi_fill_fn fill, void *f
         st.h2d_bytes += (double)input_bytes(p, b.weights != nullptr, b.flags != nullptr);
         LOOP_TRY(cudaStreamWaitEvent(p->s_compute, p->ev_h2d_done[slot], 0));
         LOOP_TRY(cudaEventRecord(p->ev_c_start[slot], p->s_compute));
-        LOOP_TRY(cudaEventRecord(p->ev[EV_START], p->s_compute));
-        LOOP_TRY(cudaEventRecord(p->ev[EV_H2D], p->s_compute));
+        if (want_info) {
+            LOOP_TRY(cudaEventRecord(p->ev[EV_START], p->s_compute));
+            LOOP_TRY(cudaEventRecord(p->ev[EV_H2D], p->s_compute));
+        }
         float *img = nullptr;
-        rc = enqueue_imaging(p, in, p->s_compute, &img);
+        rc = enqueue_imaging(p, in, p->s_compute, &img, want_info != 0);
         if (rc) break;
         LOOP_TRY(cudaEventRecord(p->ev_c_done[slot], p->s_compute));
         used[slot] = true;

@@ -48,6 +48,12 @@ class GpuImager:
         img = toi.toi_copy_image_to_host(self.plan, ptr, self.N).numpy()
         return img, info.as_dict(), rc
 
+    def image_untimed(self):
+        """The call without `info`: no per-stage timing events, no synchronisation inside the call."""
+        ptr, _, rc = toi.toi_image_snapshot(self.plan, self.t["uvw_m"], self.t["vis"], self.t["weights"],
+                                            self.t["flags"], want_info=False)
+        return toi.toi_copy_image_to_host(self.plan, ptr, self.N).numpy(), rc
+
     def indices(self):
         iu, iv = toi.toi_debug_cell_indices(self.plan, self.n_b, self.n_c)
         return iu.cpu().numpy(), iv.cpu().numpy()

@@ -269,6 +269,24 @@ def test_back_to_back_snapshots_find_a_zero_grid():
             _assert_image(img, img_o, "repeat")
 
 
+@pytest.mark.parametrize("weighting", ["natural", "uniform"])
+def test_calls_without_info_give_the_same_image(weighting):
+    """A call without `info` records no per-stage events and does not synchronise; several of them back to
+    back, then a timed one, all against the oracle's image."""
+    wl = _reduced2(n_ant=12, n_chan=130, image_size=256)
+    snap = snapshot_np(wl)
+    rc, img_o, _, _ = _oracle(snap, wl.image_size, wl.cell_size_deg, weighting, pol_a=0, pol_b=3)
+    assert rc == 0
+    with GpuImager(snap, wl.image_size, wl.cell_size_deg, weighting, pol_a=0, pol_b=3) as gi:
+        for k in range(3):
+            img, rc_g = gi.image_untimed()
+            assert rc_g == 0
+            _assert_image(img, img_o, f"untimed call {k}")
+        img, info, _ = gi.image()
+        _assert_image(img, img_o, "timed call after untimed ones")
+        assert info["ms_grid"] > 0.0 and info["ms_fft"] > 0.0
+
+
 def test_edge_non_default_grid_size():
     wl = synth.CONFIG1
     snap = snapshot_np(wl)
