@@ -27,6 +27,8 @@ __global__ void __launch_bounds__(256)
 k_clear_tiles(float2 *__restrict__ grid, float *__restrict__ dens, int G, uint8_t *__restrict__ map, int tpr,
               long long n_tiles)
 {
+    pdl_wait();
+    pdl_trigger();
     const int lane = threadIdx.x & 31;
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const long long t0 = warp * kTilesPerWarp;
@@ -71,7 +73,7 @@ void launch_clear_tiles(float2 *d_grid, float *d_density, int G, uint8_t *d_map,
     const int tpr = tiles_per_row(G);
     const long long n_tiles = (long long)tpr * tile_rows(G);
     const long long warps = (n_tiles + kTilesPerWarp - 1) / kTilesPerWarp;
-    k_clear_tiles<<<(unsigned)((warps + 7) / 8), 256, 0, stream>>>(d_grid, d_density, G, d_map, tpr, n_tiles);
+    launch_pdl(k_clear_tiles, dim3((unsigned)((warps + 7) / 8)), dim3(256), 0, stream, d_grid, d_density, G, d_map, tpr, n_tiles);
 }
 
 }  // namespace toi

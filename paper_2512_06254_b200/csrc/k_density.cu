@@ -17,6 +17,8 @@ template <bool FAST>
 __global__ void __launch_bounds__(256)
 k_density(Geometry g, Inputs in, const SnapState *__restrict__ st, float *__restrict__ D)
 {
+    pdl_wait();
+    pdl_trigger();
     if (st->status != TOI_OK) return;
     const int lane = threadIdx.x & 31;
     const int per_row = (g.n_c + 32 * kChunks - 1) / (32 * kChunks);
@@ -98,9 +100,9 @@ void launch_density(const Geometry &g, const Inputs &in, SnapState *st, float *d
     const long long blocks = (warps * 32 + threads - 1) / threads;
     const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags;
     if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
-        k_density<true><<<(unsigned)blocks, threads, 0, stream>>>(g, in, st, d_density);
+        launch_pdl(k_density<true>, dim3((unsigned)blocks), dim3(threads), 0, stream, g, in, (const SnapState *)st, d_density);
     else
-        k_density<false><<<(unsigned)blocks, threads, 0, stream>>>(g, in, st, d_density);
+        launch_pdl(k_density<false>, dim3((unsigned)blocks), dim3(threads), 0, stream, g, in, (const SnapState *)st, d_density);
 }
 
 }  // namespace toi

@@ -56,7 +56,9 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
     extern __shared__ float2 s_dyn[];
     float2 *const s_tab = s_dyn, *const s_seq = s_dyn + P::kTabFloat2;
     const int t = threadIdx.x, half = N >> 1;
-    fft::fill_tables<LOG2G>(s_tab, tw, t, T);
+    fft::fill_tables<LOG2G>(s_tab, tw, t, T);      // plan constants: before the wait, under the previous kernel's tail
+    pdl_wait();
+    pdl_trigger();
     static_assert(kTiles <= 128, "a row's tile marks are carried as two 64-bit masks");
     for (int y = blockIdx.x; y < G; y += gridDim.x) {
         const uint8_t *mrow = map + (size_t)(y / kTileH) * tiles_per_row(G);
@@ -108,7 +110,9 @@ k_fft_cols(const float2 *__restrict__ work, int N, const float2 *__restrict__ tw
     extern __shared__ float2 s_dyn[];
     float2 *const s_tab = s_dyn, *const s_seq = s_dyn + P::kTabFloat2;       // [C][SEQ]
     const int tid = threadIdx.x, half = N >> 1;
-    fft::fill_tables<LOG2G>(s_tab, tw, tid, NT);
+    fft::fill_tables<LOG2G>(s_tab, tw, tid, NT);   // plan constants: before the wait, under the previous kernel's tail
+    pdl_wait();
+    pdl_trigger();
     const double wsum = st->wsum;
     const bool ok = st->status == TOI_OK && wsum > 0.0;
     const double inv_norm = ok ? 1.0 / ((apply_jacobian ? st->omega : 1.0) * wsum) : 0.0;
@@ -174,7 +178,7 @@ void rows_launch(const float2 *grid, float2 *work, const uint8_t *map, int N, co
     if (per_sm < 1) per_sm = 1;
     int ctas = per_sm * n_sms;
     if (ctas > G) ctas = G;
-    k_fft_rows<LOG2G, T, MINB><<<ctas, T, smem, stream>>>(grid, work, map, N, tw);
+    launch_pdl(k_fft_rows<LOG2G, T, MINB>, dim3(ctas), dim3(T), smem, stream, grid, work, map, N, tw);
 }
 
 template <int LOG2G, int C, int CT, int T, int UA>
@@ -191,11 +195,11 @@ void cols_launch(const float2 *work, int N, const float2 *tw, const double *ipsi
     if (image) {
         static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, UA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        k_fft_cols<LOG2G, C, CT, T, UA, true><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image, moment);
+        launch_pdl(k_fft_cols<LOG2G, C, CT, T, UA, true>, dim3(ctas), dim3(T * CT), smem, stream, work, N, tw, ipsi, st, apply_jacobian, image, moment);
     } else {
         static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, UA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        k_fft_cols<LOG2G, C, CT, T, UA, false><<<ctas, T * CT, smem, stream>>>(work, N, tw, ipsi, st, apply_jacobian, image, moment);
+        launch_pdl(k_fft_cols<LOG2G, C, CT, T, UA, false>, dim3(ctas), dim3(T * CT), smem, stream, work, N, tw, ipsi, st, apply_jacobian, image, moment);
     }
 }
 

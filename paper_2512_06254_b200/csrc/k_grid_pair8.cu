@@ -49,6 +49,8 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
 {
     static_assert(!(PIPE && CHEB), "the Chebyshev pass computes the cell in place");
     __shared__ uint4 s_rec[kWarps * kWarpQuads];
+    pdl_wait();
+    pdl_trigger();
     if (st->status != TOI_OK) return;
     const bool has_w = OPT >= 0 ? (OPT & kHasW) != 0 : in.weights != nullptr;
     const bool has_f = OPT >= 0 ? (OPT & kHasF) != 0 : in.flags != nullptr;
@@ -280,7 +282,7 @@ template <int MODE>
 void launch_mode(int opt, dim3 grid, dim3 block, cudaStream_t stream, const Geometry &g, const Inputs &in,
                  SnapState *st, const float *D, float2 *d_grid, uint8_t *tiles, const TaskShape &shape)
 {
-#define TOI_LAUNCH(O, P) k_grid_pair8<MODE, O, P, false><<<grid, block, 0, stream>>>(g, in, st, D, d_grid, tiles, shape, ChebArgs())
+#define TOI_LAUNCH(O, P) launch_pdl(k_grid_pair8<MODE, O, P, false>, grid, block, 0, stream, g, in, st, D, d_grid, tiles, shape, ChebArgs())
     switch (opt) {
     case kHasW | kHasF | kHasD: TOI_LAUNCH(kHasW | kHasF | kHasD, true); break;
     case kHasW | kHasF: TOI_LAUNCH(kHasW | kHasF, false); break;
@@ -345,7 +347,7 @@ void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, 
     const TaskShape shape = task_shape(g, n_sms, ctas_per_sm(false), &ctas);
     const dim3 grid((unsigned)ctas), block(kWarps * 32);
     const uintptr_t aw = (uintptr_t)in.weights, af = (uintptr_t)in.flags, av = (uintptr_t)in.vis;
-#define TOI_LAUNCH_CHEB(M) k_grid_pair8<M, -1, false, true><<<grid, block, 0, stream>>>(g, in, st, d_density, d_grid, tiles, shape, cheb)
+#define TOI_LAUNCH_CHEB(M) launch_pdl(k_grid_pair8<M, -1, false, true>, grid, block, 0, stream, g, in, st, d_density, d_grid, tiles, shape, cheb)
     if (g.n_p == 4 && g.pol_a == 0 && g.pol_b == 3 && (aw & 15) == 0 && (af & 3) == 0)
         TOI_LAUNCH_CHEB(4);
     else if (g.n_p == 2 && g.pol_a == 0 && g.pol_b == 1 && (av & 15) == 0 && (aw & 7) == 0 && (af & 1) == 0)

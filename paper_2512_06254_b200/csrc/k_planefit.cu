@@ -61,6 +61,8 @@ k_planefit(int n_b, int n_c, const double *__restrict__ uvw, double S1, double S
 {
     __shared__ double red[9][kFitThreads];
     const int tid = threadIdx.x;
+    pdl_wait();                                  // the previous snapshot's last kernel still reads SnapState
+    pdl_trigger();
     double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     if (!V_inject) {
         for (int j = tid; j < n_b; j += kFitThreads) {
@@ -143,7 +145,7 @@ __global__ void k_cell_indices(Geometry g, const double *__restrict__ uvw, const
 void launch_planefit(const Geometry &g, const double *d_uvw, double S1, double S2, const double *d_V_inject,
                      SnapState *st, cudaStream_t stream)
 {
-    k_planefit<<<1, kFitThreads, 0, stream>>>(g.n_b, g.n_c, d_uvw, S1, S2, d_V_inject, st);
+    launch_pdl(k_planefit, dim3(1), dim3(kFitThreads), 0, stream, g.n_b, g.n_c, d_uvw, S1, S2, d_V_inject, st);
 }
 
 void launch_cell_indices(const Geometry &g, const double *d_uvw, const SnapState *st, int32_t *d_iu,

@@ -798,6 +798,11 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     }
     const int n_passes = slabs_run * K;
     bool have_comb[2] = {false, false};
+    struct PdlOff {                              // no programmatic launches while two lanes share the SMs
+        bool saved;
+        explicit PdlOff(bool off) : saved(g_pdl_enabled) { if (off) g_pdl_enabled = false; }
+        ~PdlOff() { g_pdl_enabled = saved; }
+    } pdl_off(two_lanes);
     for (int pass = 0; pass < n_passes; ++pass) {
         const int sp = pass / K, k = pass % K;
         const int L = two_lanes ? (k & 1) : 0;
