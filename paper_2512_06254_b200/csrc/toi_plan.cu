@@ -38,7 +38,9 @@ struct toi_plan {
     size_t n_samples = 0, n_elems = 0;
 
     double *d_s = nullptr, *d_ipsi = nullptr, *d_V_inject = nullptr, *d_V_reproject = nullptr;
-    SnapState *d_state = nullptr, *h_state = nullptr;
+    SnapState *d_state = nullptr, *h_state = nullptr;    // d_state: the current snapshot's, one of
+    SnapState *d_state_slots = nullptr;                  // two slots taken in turn: the plane fit of snapshot n + 1
+    unsigned state_pos = 0;                              // writes its slot while snapshot n's last kernel reads the other
     DevSlot dev_in[2];
     toi_snapshot_buffers pin[2] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
     // ONE gridding grid (with guard band) and ONE density map, both zero between snapshots: the
@@ -53,7 +55,9 @@ struct toi_plan {
     bool s_monotone = true;      // channel scales monotone: the gridder can bound a strip's tiles by its ends
     float2 *d_grid_keep = nullptr;                       // cfg.debug_keep_grid
     float *d_dens_keep = nullptr;
-    cudaEvent_t ev_done = nullptr;                       // end of the last imaging call (any stream)
+    cudaEvent_t ev_done = nullptr;                       // end of the last imaging call, recorded only when the next
+    cudaStream_t last_stream = nullptr;                  // call comes on ANOTHER stream than last_stream (an event
+    bool have_last = false;                              // record between two kernels would break their launch overlap)
     cudaEvent_t ev_clear0 = nullptr, ev_clear1 = nullptr;
     float *d_images = nullptr;
     int ring_depth = 5;
@@ -173,7 +177,7 @@ int free_plan(toi_plan *p)
     if (p->s_copy) cudaStreamSynchronize(p->s_copy);
     if (p->fft_ok) cufftDestroy(p->fft);
     if (p->fft_pruned) { cufftDestroy(p->fft_cols); cufftDestroy(p->fft_rows); }
-    cudaFree(p->d_s); cudaFree(p->d_ipsi); cudaFree(p->d_V_inject); cudaFree(p->d_V_reproject); cudaFree(p->d_state);
+    cudaFree(p->d_s); cudaFree(p->d_ipsi); cudaFree(p->d_V_inject); cudaFree(p->d_V_reproject); cudaFree(p->d_state_slots);
     cudaFreeHost(p->h_state);
     for (int k = 0; k < 2; ++k) {
         cudaFree(p->dev_in[k].uvw); cudaFree(p->dev_in[k].vis);
@@ -235,6 +239,24 @@ int set_fft_stream(toi_plan *p, cudaStream_t stream)
                           cufftSetStream(p->fft_rows, stream) != CUFFT_SUCCESS))
         return fail(p, TOI_ERR_CUFFT, "cufftSetStream failed");
     p->fft_stream = stream;
+    return TOI_OK;
+}
+
+// One grid, one workspace: a call on another stream than the previous call's waits for that call's last
+// kernel; on the same stream the stream order already says so.  Also takes the next SnapState slot.
+int follow_previous_call(toi_plan *p, cudaStream_t stream)
+{
+    if (p->have_last && p->last_stream != stream) {
+        if (cudaEventRecord(p->ev_done, p->last_stream) == cudaSuccess) {
+            CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_done, 0));
+        } else {                                 // the caller destroyed that stream: its work is done or draining
+            cudaGetLastError();
+            CU_TRY(p, cudaDeviceSynchronize());
+        }
+    }
+    p->last_stream = stream;
+    p->have_last = true;
+    p->d_state = p->d_state_slots + (++p->state_pos & 1u);       // this snapshot's SnapState
     return TOI_OK;
 }
 
@@ -305,8 +327,8 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     int launches = 0;
     int rc = set_fft_stream(p, stream);
     if (rc) return rc;
-    // one grid, one workspace: a call on another stream waits for the previous call's last kernel
-    CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_done, 0));
+    rc = follow_previous_call(p, stream);
+    if (rc) return rc;
     const bool uniform = p->cfg.weighting == TOI_WEIGHT_UNIFORM;
     // a1-a2: plane fit (also resets the per-snapshot accumulators)
     launch_planefit(g, in.uvw, p->S1, p->S2, p->inject ? p->d_V_inject : nullptr, p->d_state, stream);
@@ -341,7 +363,6 @@ int enqueue_imaging(toi_plan *p, const Inputs &in, cudaStream_t stream, float **
     rc = transform_and_clear(p, stream, p->d_grid, p->d_tiles_grid, p->d_work, uniform, timed, img, 0, nullptr, &launches);
     if (rc) return rc;
     if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_CROP], stream));
-    CU_TRY(p, cudaEventRecord(p->ev_done, stream));
     CU_TRY(p, cudaGetLastError());
     p->last_in = in;
     p->last_launches = launches;
@@ -512,8 +533,9 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     CREATE_TRY(cudaMemcpy(p->d_ipsi, ipsi.data(), (size_t)N * sizeof(double), cudaMemcpyHostToDevice));
     CREATE_TRY(cudaMalloc(&p->d_V_inject, 9 * sizeof(double)));
     CREATE_TRY(cudaMalloc(&p->d_V_reproject, 9 * sizeof(double)));
-    CREATE_TRY(cudaMalloc(&p->d_state, sizeof(SnapState)));
-    CREATE_TRY(cudaMemset(p->d_state, 0, sizeof(SnapState)));
+    CREATE_TRY(cudaMalloc(&p->d_state_slots, 2 * sizeof(SnapState)));
+    CREATE_TRY(cudaMemset(p->d_state_slots, 0, 2 * sizeof(SnapState)));
+    p->d_state = p->d_state_slots;
     CREATE_TRY(cudaMallocHost(&p->h_state, sizeof(SnapState)));
     // the gridding grid with a guard band on both sides (the gridder's 8 x 8 window may overhang the
     // grid by one row or column of zero accumulators, whose flush must land in owned memory that
@@ -530,7 +552,6 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
         CREATE_TRY(cudaMemset(p->d_dens, 0, GG * sizeof(float)));
     }
     CREATE_TRY(cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming));
-    CREATE_TRY(cudaEventRecord(p->ev_done, p->s_compute));
     CREATE_TRY(cudaEventCreate(&p->ev_clear0));
     CREATE_TRY(cudaEventCreate(&p->ev_clear1));
     if (cfg->debug_keep_grid) {
@@ -722,7 +743,8 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     const size_t GG = (size_t)g.G * g.G, NN = (size_t)g.N * g.N;
     int rc = set_fft_stream(p, stream);
     if (rc) return rc;
-    CU_TRY(p, cudaStreamWaitEvent(stream, p->ev_done, 0));
+    rc = follow_previous_call(p, stream);
+    if (rc) return rc;
     CU_TRY(p, cudaEventRecord(p->ev3_a, stream));
     Inputs in;
     if (p->cfg.input_location == TOI_MEM_HOST) {
@@ -744,7 +766,6 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     p->last_in = in;
     if (p->h_state->status != TOI_OK) {
         CU_TRY(p, cudaMemsetAsync(img, 0, NN * sizeof(float), stream));
-        CU_TRY(p, cudaEventRecord(p->ev_done, stream));
         return fail(p, p->h_state->status, "degenerate geometry: the snapshot's baselines do not span a plane (or V33 < 1e-6)");
     }
     const double beta = p->cfg.cell_size_deg * (3.14159265358979323846 / 180.0);
@@ -754,7 +775,6 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     const int n_slab = n_slab_in > 0 ? n_slab_in : (int)fmax(1.0, ceil(phi_max / 10.0));          // Eq. 27
     if (n_slab > 1024) {
         CU_TRY(p, cudaMemsetAsync(img, 0, NN * sizeof(float), stream));
-        CU_TRY(p, cudaEventRecord(p->ev_done, stream));
         return fail(p, TOI_ERR_UNSUPPORTED, "more than 1024 slabs: the snapshot is far from coplanar");
     }
     const double alpha_slab = phi_max / n_slab;
@@ -850,7 +870,6 @@ int toi_image_snapshot_3d(toi_plan *p, const double *uvw_m, const void *vis, con
     launch_cheb_finish(g.N, beta, p->d_state, p->apply_jacobian, p->d_acc3, img, stream);
     ++launches;
     CU_TRY(p, cudaEventRecord(p->ev3_b, stream));
-    CU_TRY(p, cudaEventRecord(p->ev_done, stream));
     CU_TRY(p, cudaGetLastError());
     p->last_launches = launches;
     if (info3 || info) {
