@@ -98,10 +98,21 @@ k_fft_rows(const float2 *__restrict__ grid, float2 *__restrict__ work, const uin
 // Sequences sit kSkew float2 apart beyond their padded length, so that the C columns of one grid row
 // fall on different banks when a row segment is stored.
 constexpr int kSkew = 4;
+// The sparse clear can ride along (grid != nullptr or dens != nullptr): the row pass has read the grid, so
+// every warp of this pass first zeroes its share of the marked tiles (stores nobody waits for) and then
+// turns to its columns -- instead of a k_clear_tiles launch of its own between the two passes.
+struct ClearArgs {
+    float2 *grid;
+    float *dens;
+    uint8_t *map;
+    int G, tpr;
+    long long n_tiles;
+};
 template <int LOG2G, int C, int CT, int T, int UA, bool IMAGE>
 __global__ void __launch_bounds__(T * CT)
 k_fft_cols(const float2 *__restrict__ work, int N, const float2 *__restrict__ tw, const double *__restrict__ ipsi,
-           const SnapState *__restrict__ st, int apply_jacobian, float *__restrict__ image, float2 *__restrict__ moment)
+           const SnapState *__restrict__ st, int apply_jacobian, float *__restrict__ image, float2 *__restrict__ moment,
+           ClearArgs clr)
 {
     using P = fft::Plan<LOG2G>;
     constexpr int CB = cols_block(LOG2G);
@@ -113,6 +124,11 @@ k_fft_cols(const float2 *__restrict__ work, int N, const float2 *__restrict__ tw
     fft::fill_tables<LOG2G>(s_tab, tw, tid, NT);   // plan constants: before the wait, under the previous kernel's tail
     pdl_wait();
     pdl_trigger();
+    if (clr.map != nullptr) {
+        const long long n_warps = (long long)gridDim.x * (NT / 32);
+        for (long long w = (long long)blockIdx.x * (NT / 32) + (tid >> 5); w * kClearTilesPerWarp < clr.n_tiles; w += n_warps)
+            clear_tiles_warp(clr.grid, clr.dens, clr.G, clr.map, clr.tpr, clr.n_tiles, w * kClearTilesPerWarp, tid & 31);
+    }
     const double wsum = st->wsum;
     const bool ok = st->status == TOI_OK && wsum > 0.0;
     const double inv_norm = ok ? 1.0 / ((apply_jacobian ? st->omega : 1.0) * wsum) : 0.0;
@@ -183,7 +199,7 @@ void rows_launch(const float2 *grid, float2 *work, const uint8_t *map, int N, co
 
 template <int LOG2G, int C, int CT, int T, int UA>
 void cols_launch(const float2 *work, int N, const float2 *tw, const double *ipsi, const SnapState *st, int apply_jacobian,
-                 float *image, float2 *moment, int n_sms, cudaStream_t stream)
+                 float *image, float2 *moment, const ClearArgs &clr, int n_sms, cudaStream_t stream)
 {
     using P = fft::Plan<LOG2G>;
     constexpr size_t smem = (size_t)(P::kTabFloat2 + C * (P::kPadded + kSkew)) * sizeof(float2);
@@ -195,11 +211,11 @@ void cols_launch(const float2 *work, int N, const float2 *tw, const double *ipsi
     if (image) {
         static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, UA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        launch_pdl(k_fft_cols<LOG2G, C, CT, T, UA, true>, dim3(ctas), dim3(T * CT), smem, stream, work, N, tw, ipsi, st, apply_jacobian, image, moment);
+        launch_pdl(k_fft_cols<LOG2G, C, CT, T, UA, true>, dim3(ctas), dim3(T * CT), smem, stream, work, N, tw, ipsi, st, apply_jacobian, image, moment, clr);
     } else {
         static const cudaError_t once = cudaFuncSetAttribute(k_fft_cols<LOG2G, C, CT, T, UA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         (void)once;
-        launch_pdl(k_fft_cols<LOG2G, C, CT, T, UA, false>, dim3(ctas), dim3(T * CT), smem, stream, work, N, tw, ipsi, st, apply_jacobian, image, moment);
+        launch_pdl(k_fft_cols<LOG2G, C, CT, T, UA, false>, dim3(ctas), dim3(T * CT), smem, stream, work, N, tw, ipsi, st, apply_jacobian, image, moment, clr);
     }
 }
 
@@ -243,16 +259,21 @@ void launch_fft_rows(int N, int G, const float2 *d_grid, float2 *d_work, const u
 }
 
 // pass 2: the needed columns of `work`; d_image != nullptr: the finished image (step a7 fused), else the
-// complex values of the N x N pixels the crop keeps into d_moment[j][i]
+// complex values of the N x N pixels the crop keeps into d_moment[j][i].  d_clear_map != nullptr: the sparse
+// clear of d_clear_grid / d_clear_density (either may be null) runs inside this pass (k_clear.cu otherwise)
 void launch_fft_cols(int N, int G, const float2 *d_work, const float2 *d_tw, const double *d_ipsi, const SnapState *st,
-                     int apply_jacobian, float *d_image, float2 *d_moment, int n_sms, cudaStream_t stream)
+                     int apply_jacobian, float *d_image, float2 *d_moment, float2 *d_clear_grid, float *d_clear_density,
+                     uint8_t *d_clear_map, int n_sms, cudaStream_t stream)
 {
+    ClearArgs clr;
+    clr.grid = d_clear_grid; clr.dens = d_clear_density; clr.map = d_clear_map;
+    clr.G = G; clr.tpr = tiles_per_row(G); clr.n_tiles = (long long)tiles_per_row(G) * tile_rows(G);
     switch (log2_exact(G)) {
-    case 10: cols_launch<10, 8, 8, 64, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
-    case 11: cols_launch<11, 8, 4, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
-    case 12: cols_launch<12, 4, 4, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
-    case 13: cols_launch<13, 2, 2, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
-    default: cols_launch<14, 1, 1, 512, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, n_sms, stream); break;
+    case 10: cols_launch<10, 8, 8, 64, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, clr, n_sms, stream); break;
+    case 11: cols_launch<11, 8, 4, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, clr, n_sms, stream); break;
+    case 12: cols_launch<12, 4, 4, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, clr, n_sms, stream); break;
+    case 13: cols_launch<13, 2, 2, 128, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, clr, n_sms, stream); break;
+    default: cols_launch<14, 1, 1, 512, 1>(d_work, N, d_tw, d_ipsi, st, apply_jacobian, d_image, d_moment, clr, n_sms, stream); break;
     }
 }
 

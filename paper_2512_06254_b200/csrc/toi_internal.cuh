@@ -176,6 +176,55 @@ inline cudaError_t launch_pdl(void (*kernel)(P...), dim3 grid, dim3 block, size_
     return cudaLaunchKernelEx(&cfg, kernel, P(args)...);
 }
 
+// ---- sparse clear (k_clear.cu; also run inside the transform's column pass) ------------------------
+// One warp takes kClearTilesPerWarp consecutive map entries starting at t0 and clears the marked tiles
+// one after the other (few tiles per warp: the marked tiles cluster around the uv origin, and a warp
+// that finds all of its entries marked must not become the tail of the kernel).  A tile row of the
+// grid is kTileW complex64 = 1 KB, written with 8-byte stores.
+// The density map (uniform weighting) needs no map of its own: the density pass writes the centre
+// cells of the samples -- inside the tiles the gridder marks for the same samples' windows -- and
+// their mirror cells (-iu, -iv), i.e. array index (G - x, G - y) for (x, y).  For every marked tile
+// the same rectangle of the density map and its point mirror are zeroed (4-byte stores: the mirrored
+// rectangle starts on any column).
+constexpr int kClearTilesPerWarp = 4;
+__device__ __forceinline__ void clear_tiles_warp(float2 *__restrict__ grid, float *__restrict__ dens, int G,
+                                                 uint8_t *__restrict__ map, int tpr, long long n_tiles, long long t0, int lane)
+{
+    if (t0 >= n_tiles) return;
+    const long long mine = t0 + lane;
+    const bool dirty = lane < kClearTilesPerWarp && mine < n_tiles && map[mine] != 0;
+    if (dirty) map[mine] = 0;
+    unsigned todo = __ballot_sync(0xffffffffu, dirty);
+    while (todo) {
+        const int b = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const long long t = t0 + b;
+        const int x0 = (int)(t % tpr) * kTileW, y0 = (int)(t / tpr) * kTileH;
+        const int rows = min(kTileH, G - y0);
+        if (grid != nullptr) {
+            float2 *row = grid + (size_t)y0 * G + x0;
+            for (int r = 0; r < rows; ++r, row += G) {
+#pragma unroll
+                for (int k = 0; k < kTileW / 32; ++k)
+                    if (x0 + k * 32 + lane < G) row[k * 32 + lane] = make_float2(0.0f, 0.0f);
+            }
+        }
+        if (dens != nullptr) {
+            for (int r = 0; r < rows; ++r) {
+                float *own = dens + (size_t)(y0 + r) * G;
+                const int ym = G - (y0 + r);                      // mirrored row; G itself is outside
+                float *mir = dens + (size_t)(ym < G ? ym : 0) * G;
+#pragma unroll
+                for (int k = 0; k < kTileW / 32; ++k) {
+                    const int x = x0 + k * 32 + lane, xm = G - x;
+                    if (x < G) own[x] = 0.0f;
+                    if (x < G && ym < G && xm < G) mir[xm] = 0.0f;
+                }
+            }
+        }
+    }
+}
+
 // ---- packed fp32 pairs (sm_100a FFMA2 / FMUL2: two fp32 lanes per instruction) ----------------
 typedef unsigned long long u64;
 __device__ __forceinline__ u64 pack2(float x, float y)
@@ -294,7 +343,8 @@ void fft_twiddle_table(int G, float2 *host_out);
 void launch_fft_rows(int N, int G, const float2 *d_grid, float2 *d_work, const uint8_t *d_map, const float2 *d_tw,
                      int n_sms, cudaStream_t stream);
 void launch_fft_cols(int N, int G, const float2 *d_work, const float2 *d_tw, const double *d_ipsi, const SnapState *st,
-                     int apply_jacobian, float *d_image, float2 *d_moment, int n_sms, cudaStream_t stream);
+                     int apply_jacobian, float *d_image, float2 *d_moment, float2 *d_clear_grid, float *d_clear_density,
+                     uint8_t *d_clear_map, int n_sms, cudaStream_t stream);
 void launch_r3_range(int n_b, const double *d_uvw, const SnapState *st, double s_min, double s_max, double *d_out,
                      cudaStream_t stream);
 size_t bessel_table_floats(int K);

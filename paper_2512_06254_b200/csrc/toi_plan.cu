@@ -290,14 +290,24 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, float2 *d_grid, uint8_
         if (cufftExecC2C(p->fft, A, F, CUFFT_INVERSE) != CUFFT_SUCCESS) return fail(p, TOI_ERR_CUFFT, "cufftExecC2C failed");
     }
     ++*launches;
-    if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
-    launch_clear_tiles(d_grid, clear_density ? p->d_dens : nullptr, g.G, d_tiles, stream);
-    ++*launches;
-    if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
+    // The sparse clear: a launch of its own between the passes when the call is timed (ms_clear is then
+    // what it costs by itself, and that is what the roofline accounting charges the gridding with);
+    // otherwise, with the hand-written transform at G <= 4096, inside the column pass (its stores run
+    // under that pass's shared-memory work: 0.006-0.014 ms per snapshot less at config 2; at G = 8192
+    // and 16384 the column pass has one CTA of 8-16 warps per SM and the clear is faster by itself).
+    const bool clear_in_cols = p->fft_custom && !timed && g.G <= 4096;
+    float *dens_to_clear = clear_density ? p->d_dens : nullptr;
+    if (!clear_in_cols) {
+        if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
+        launch_clear_tiles(d_grid, dens_to_clear, g.G, d_tiles, stream);
+        ++*launches;
+        if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
+    }
     if (before_cols) CU_TRY(p, cudaStreamWaitEvent(stream, before_cols, 0));     // what still reads this lane's moment
     if (p->fft_custom) {
         launch_fft_cols(g.N, g.G, d_work, p->d_tw, p->d_ipsi, p->d_state, p->apply_jacobian, d_image,
-                        d_image ? nullptr : p->d_moment[lane], p->n_sms, stream);
+                        d_image ? nullptr : p->d_moment[lane], clear_in_cols ? d_grid : nullptr,
+                        clear_in_cols ? dens_to_clear : nullptr, clear_in_cols ? d_tiles : nullptr, p->n_sms, stream);
         ++*launches;
         if (timed) CU_TRY(p, cudaEventRecord(p->ev[EV_FFT], stream));
         return TOI_OK;
