@@ -284,6 +284,33 @@ int toi_debug_copy_grid(toi_plan *plan, void *d_grid_c64);
 /* Uniform-weighting density of the LAST snapshot, float32 [G][G], same index convention. */
 int toi_debug_copy_density(toi_plan *plan, float *d_density);
 
+/* ---- allocation-free entry point ------------------------------------------------------------ */
+/* Steps a1-a3 (DESIGN.md section 3 steps 1-5) without a plan and WITHOUT ANY ALLOCATION,
+ * for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): plane fit of the snapshot's baselines, rotation, and the centre cell of every
+ * (baseline, channel) sample -- bit-identical to what a plan computes (toi_debug_cell_indices).
+ *   d_uvw_m       DEVICE, f64 [n_baselines][3], metres
+ *   chan_freq_hz  HOST, f64 [n_channels], Hz, positive; n_channels <= TOI_STATIC_MAX_CHANNELS
+ *                 (TOI_ERR_UNSUPPORTED beyond it: the scratch is a fixed-size array)
+ *   grid_size     G in [2, 32768]; cell_size_deg the image cell, degrees
+ *   cuda_stream   cudaStream_t or NULL; the work is enqueued on it, the call does not synchronise
+ *                 (the copy of the channel table from pageable host memory may wait for the stream's
+ *                 earlier work)
+ *   d_iu, d_iv    DEVICE out, int32 [n_baselines][n_channels]: signed centre cells (TOI off-grid
+ *                 samples keep their out-of-range index, as in toi_debug_cell_indices)
+ *   d_fit_out     DEVICE out or NULL: 13 doubles, V[9] row-major, omega (Eq. 8), singular values[3]
+ *   err, err_len  NULL / 0, or a buffer the error text is written to
+ * The scratch (snapshot state + channel scale table, 256 B + 8 B x TOI_STATIC_MAX_CHANNELS) is a
+ * file-scope __device__ array: every GPU that loads the library holds it until the process exits.
+ * All calls share it and it keeps the last call's contents (nothing in it needs to start at zero: each
+ * call rewrites what it reads).  Calls that OVERLAP ON THE GPU -- different streams, or several host
+ * threads on one device -- race on it; calls on one stream are ordered by the stream.
+ * Calls no cudaMalloc / cudaFree / allocating library routine.  Returns TOI_OK or an error < 0. */
+#define TOI_STATIC_MAX_CHANNELS 32768
+int toi_cell_indices_static(const double *d_uvw_m, int32_t n_baselines, const double *chan_freq_hz,
+                            int32_t n_channels, int32_t grid_size, double cell_size_deg, void *cuda_stream,
+                            int32_t *d_iu, int32_t *d_iv, double *d_fit_out, char *err, int32_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

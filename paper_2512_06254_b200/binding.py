@@ -27,7 +27,7 @@ EXPORTS = ["toi_plan_create", "toi_plan_destroy", "toi_image_snapshot", "toi_pla
            "toi_reproject", "toi_difference",
            "toi_last_error", "toi_last_launch_count",
            "toi_debug_set_transform", "toi_debug_cell_indices", "toi_debug_keep_grid",
-           "toi_debug_copy_grid", "toi_debug_copy_density"]
+           "toi_debug_copy_grid", "toi_debug_copy_density", "toi_cell_indices_static"]
 
 
 class toi_config(C.Structure):
@@ -318,6 +318,24 @@ def toi_debug_cell_indices(plan, n_baselines, n_channels, device="cuda"):
     iv = torch.empty_like(iu)
     _check(plan, load().toi_debug_cell_indices(plan, _ptr(iu), _ptr(iv)))
     return iu, iv
+
+
+TOI_STATIC_MAX_CHANNELS = 32768
+
+
+def toi_cell_indices_static(uvw_m, chan_freq_hz, grid_size, cell_size_deg, iu, iv, fit_out=None, stream=None):
+    """Steps a1-a3 without a plan and without any allocation (include/toi.h): fills the caller's device
+    tensors iu, iv (int32 [n_baselines][n_channels]) and, if given, fit_out (float64 [13]: V, omega, sing)."""
+    lib = load()
+    freq = torch.as_tensor(chan_freq_hz, dtype=torch.float64, device="cpu").contiguous()
+    err = C.create_string_buffer(256)
+    st = stream if stream is not None else torch.cuda.current_stream(uvw_m.device)
+    rc = lib.toi_cell_indices_static(_ptr(uvw_m), C.c_int32(uvw_m.shape[0]), C.c_void_p(freq.data_ptr()),
+                                     C.c_int32(freq.numel()), C.c_int32(grid_size), C.c_double(cell_size_deg),
+                                     C.c_void_p(st.cuda_stream), _ptr(iu), _ptr(iv), _ptr(fit_out), err, C.c_int32(256))
+    if rc != TOI_OK:
+        raise ToiError(rc, err.value.decode(errors="replace"))
+    return rc
 
 
 def toi_debug_keep_grid(plan, on=True):

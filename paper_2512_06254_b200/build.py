@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtoi.so")
 SOURCES = ["toi_plan.cu", "k_planefit.cu", "k_density.cu", "k_grid_atomic.cu", "k_grid_pair8.cu", "k_clear.cu", "k_fft.cu",
-           "k_correct_crop.cu", "k_reproject.cu", "k_cheb.cu"]
+           "k_correct_crop.cu", "k_reproject.cu", "k_cheb.cu", "toi_static.cu"]
 HEADERS = [os.path.join(CSRC, "toi_internal.cuh"), os.path.join(CSRC, "grid_window.cuh"), os.path.join(CSRC, "fft_smem.cuh"), os.path.join(CSRC, "tap_poly.inc"),
            os.path.join(HERE, "..", "include", "toi.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
