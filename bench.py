@@ -221,6 +221,10 @@ def time_stages(toi, plan, snap, stream, reps):
     """Per-stage durations (CUDA events inside the library, on `stream`; every call synchronises)."""
     acc = {k: [] for k in STAGE_KEYS}
     info = None
+    # warm-up of the timed path itself: a call with `info` launches the sparse clear as a kernel of its own,
+    # which the untimed steps before never did (lazy module loading put 50-80 us into its first launch)
+    for _ in range(2):
+        toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"], stream=stream, want_info=True)
     for _ in range(reps):
         _, info, _ = toi.toi_image_snapshot(plan, snap["uvw_m"], snap["vis"], snap["weights"], snap["flags"],
                                             stream=stream, want_info=True)
