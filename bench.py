@@ -323,7 +323,13 @@ def run_ours(args):
     launches_per_step = toi.toi_last_launch_count(plan)
     sampler = ClockSampler(local)
     sampler.start()
-    time.sleep(0.3)
+    # the sampler needs ~0.3 s to come up; the GPU keeps working meanwhile (more untimed warm-up steps): a
+    # timed region of a few ms that starts on a GPU that has just idled measures its clock ramp, not the path
+    t_busy = time.time() + 0.3
+    while time.time() < t_busy:
+        for _ in range(50):
+            step()
+        torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     shard.barrier()
     torch.cuda.synchronize()

@@ -61,10 +61,9 @@ k_planefit(int n_b, int n_c, const double *__restrict__ uvw, double S1, double S
 {
     __shared__ double red[9][kFitThreads];
     const int tid = threadIdx.x;
-    // Nothing here reads what an earlier kernel wrote, and SnapState alternates between two slots (the
-    // previous snapshot's last kernel reads the other one): the whole fit runs under that kernel.  Thread 0
-    // waits for it just before leaving, so that "this kernel has completed" still implies "everything
-    // before it has", which is what the next kernel's wait relies on.
+    // uvw may have been produced on this stream by the caller's own kernel just before the call: wait for
+    // whatever precedes (visibility of its writes is guaranteed only behind this wait) before reading it
+    pdl_wait();
     pdl_trigger();
     double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     if (!V_inject) {
@@ -126,7 +125,6 @@ k_planefit(int n_b, int n_c, const double *__restrict__ uvw, double S1, double S
     for (int k = 0; k < 9; ++k) st->V[k] = V[k];
     st->omega = fabs(V[0] * V[4] - V[3] * V[1]);                           // Eq. 8
     if (!(V[8] >= 1e-6)) st->status = TOI_ERR_DEGENERATE_GEOMETRY;
-    pdl_wait();
 }
 
 __global__ void k_cell_indices(Geometry g, const double *__restrict__ uvw, const SnapState *__restrict__ st,

@@ -40,7 +40,7 @@ struct toi_plan {
     double *d_s = nullptr, *d_ipsi = nullptr, *d_V_inject = nullptr, *d_V_reproject = nullptr;
     SnapState *d_state = nullptr, *h_state = nullptr;    // d_state: the current snapshot's, one of
     SnapState *d_state_slots = nullptr;                  // two slots taken in turn: the plane fit of snapshot n + 1
-    unsigned state_pos = 0;                              // writes its slot while snapshot n's last kernel reads the other
+    unsigned state_pos = 0;                              // never writes what consumers of snapshot n (re-projection) read
     DevSlot dev_in[2];
     toi_snapshot_buffers pin[2] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
     // ONE gridding grid (with guard band) and ONE density map, both zero between snapshots: the
