@@ -35,6 +35,17 @@ struct TaskShape {
     unsigned t1, j1, n_tasks;       // tasks of the first kind, rows they cover, all tasks
 };
 
+// An atomic add (inline PTX included) is compiled by ptxas into its warp-aggregated form: elect a lane,
+// add the population count, broadcast the result with a shuffle -- which waits for the atomic's round
+// trip to L2 on the spot (2 % of the kernel's warp time).  atom.inc with a bound no task count reaches
+// is not rewritten: its result stays in flight until the next task needs it.
+__device__ __forceinline__ unsigned claim_task(unsigned *counter)
+{
+    unsigned t;
+    asm volatile("atom.global.inc.u32 %0, [%1], 0x7fffffff;" : "=r"(t) : "l"(counter) : "memory");
+    return t;
+}
+
 constexpr int kWarps = 8;         // warps per CTA
 constexpr int ctas_per_sm(bool) { return 2; }          // 16 warps/SM at <= 128 registers (4 x 4 warps measured 1 % slower)
 
@@ -77,16 +88,37 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
     // dynamic task queue; the NEXT task is requested while the current one is processed (the atomic's
     // round trip to L2 was 4 % of the kernel when taken in place)
     unsigned task_ahead = 0;
-    if (lane == 0) task_ahead = atomicAdd(&st->task_counter, 1u);
+    if (lane == 0) task_ahead = claim_task(&st->task_counter);
     for (;;) {
         const unsigned task = __shfl_sync(0xffffffffu, task_ahead, 0);
         if (task >= shape.n_tasks) break;
-        if (lane == 0) task_ahead = atomicAdd(&st->task_counter, 1u);
+        if (lane == 0) task_ahead = claim_task(&st->task_counter);
         const bool big = task < shape.t1;
         const unsigned t_in = big ? task : task - shape.t1, tpr = (unsigned)(big ? shape.tpr1 : shape.tpr2);
         const int strip_len = big ? shape.strip1 : shape.strip2;
         const int j = (int)((big ? 0u : shape.j1) + t_in / tpr);
         const int c_task = (int)(t_in % tpr) * (kGroups * strip_len);
+        const int c_lo = c_task + grp * strip_len + pre_k;        // my channel in batch 0
+        const int c_hi = min(c_task + (grp + 1) * strip_len, g.n_c);
+        const long long q_row = (long long)j * g.n_c;
+
+        // The task's first loads go out before anything waits: raw inputs of batch 0 (DRAM), channel
+        // scales, then the baseline (L2).  Taken one after the other -- baseline, rotation, tile marks,
+        // raw inputs -- their latencies added up to 15 % of the kernel's warp time.
+        Raw nxt;
+        nxt.a = nxt.b = make_float2(0.0f, 0.0f); nxt.wa = nxt.wb = 0.0f; nxt.fl = 0u; nxt.s = 0.0;
+        double s_first = 0.0, s_ahead = 0.0;
+        auto first_loads = [&]() {
+            if (c_lo < c_hi) {
+                load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c_lo, c_lo, nxt);
+                if (PIPE) {
+                    s_first = __ldg(g.s + c_lo);
+                    if (c_lo + kBatch < c_hi) s_ahead = __ldg(g.s + c_lo + kBatch);
+                }
+            }
+        };
+        if (!CHEB) first_loads();
+        __syncwarp();                        // keeps ptxas from hoisting the baseline's loads (and their first use) above these
         double rho1, rho2;
         rotate_baseline(st->V, in.uvw + 3 * j, rho1, rho2);
         const double rho3 = CHEB ? rotate_row3(st->V, in.uvw + 3 * j) : 0.0;
@@ -100,14 +132,14 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
             const int pb = min((int)floor((fmax(ra, rb) - cheb.r3_min) / (2.0 * cheb.d)), cheb.n_slab - 1);
             if (cheb.p < pa || cheb.p > pb) continue;
         }
-        const int c_lo = c_task + grp * strip_len + pre_k;        // my channel in batch 0
-        const int c_hi = min(c_task + (grp + 1) * strip_len, g.n_c);
-        const long long q_row = (long long)j * g.n_c;
+        if (CHEB) first_loads();
 
         // Sparse clear (k_clear.cu): mark the tiles my strip's windows can reach.  The samples of a
         // strip lie on a ray, monotone in channel (the plan passes `tiles` only when the channel
         // scales are monotone), so the windows stay inside the box spanned by the strip's two end
         // samples, widened by the 4 cells a window reaches beyond its sample's centre on either side.
+        // Plain stores, nothing read back: testing an entry first made every mark a dependent load
+        // (5 % of the kernel's warp time waiting for them).
         if (tiles != nullptr) {
             const int c_first = c_task + grp * strip_len;
             const bool some = c_first < c_hi;
@@ -122,8 +154,7 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                 const int x0 = max(min(iu, ju) - 4 + h, 0) / kTileW, x1 = min(max(iu, ju) + 4 + h, G - 1) / kTileW;
                 const int y0 = max(min(iv, jv) - 4 + h, 0) / kTileH, y1 = min(max(iv, jv) + 4 + h, G - 1) / kTileH;
                 for (int ty = y0; ty <= y1; ++ty)
-                    for (int tx = x0; tx <= x1; ++tx)
-                        if (tiles[ty * tpr + tx] == 0) tiles[ty * tpr + tx] = 1;   // L1 hit instead of a store, mostly
+                    for (int tx = x0; tx <= x1; ++tx) tiles[ty * tpr + tx] = 1;
             }
         }
 
@@ -154,18 +185,9 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
         };
         // software pipeline: raw inputs and cell (+ density) of batch b + 1 are requested while
         // batch b is processed; the channel scale s_c runs two batches ahead
-        Raw nxt;
-        nxt.a = nxt.b = make_float2(0.0f, 0.0f); nxt.wa = nxt.wb = 0.0f; nxt.fl = 0u; nxt.s = 0.0;
         Cell cnxt;
         cnxt.key = kNoKey; cnxt.sh = 0u; cnxt.xu = cnxt.xv = 0.0f; cnxt.dens = 1.0f;
-        double s_ahead = 0.0;
-        if (c_lo < c_hi) {
-            load_raw<MODE, !PIPE>(g, in, has_w, has_f, q_row + c_lo, c_lo, nxt);
-            if (PIPE) {
-                locate(__ldg(g.s + c_lo), cnxt);
-                if (c_lo + kBatch < c_hi) s_ahead = __ldg(g.s + c_lo + kBatch);
-            }
-        }
+        if (PIPE && c_lo < c_hi) locate(s_first, cnxt);
 
         for (int b = 0; b < strip_len && c_task + b < g.n_c; b += kBatch) {
             // ---------------- pre-process one sample per lane ----------------
