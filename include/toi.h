@@ -88,10 +88,12 @@ typedef struct {
     double wsum;                /* sum_q f_q w_I,q over gridded samples: Eq. 7's N_vis */
     int64_t n_gridded, n_off_grid, n_flagged;
     float ms_h2d, ms_planefit, ms_weight, ms_grid, ms_fft, ms_crop, ms_total;
-    float ms_clear;             /* sparse clear of the gridding grid (and, in the same launch, of the
-                                   density map): only the 128x8-cell tiles this snapshot touched are
-                                   zeroed again, after the first FFT pass has read the grid; not
-                                   included in ms_fft */
+    float ms_clear;             /* sparse clear of the gridding grid: only the 128x8-cell tiles this
+                                   snapshot touched are zeroed again, after the first FFT pass has
+                                   read the grid; not included in ms_fft */
+    float ms_clear_density;     /* uniform weighting: the same for the density map (the rectangles
+                                   under and opposite the marked tiles), a launch of its own in a
+                                   call that asks for this info; 0 otherwise; not included in ms_fft */
 } toi_snapshot_info;
 
 /* Allocate everything: device input slots, gridding grid, FFT workspace, tile maps, image ring,

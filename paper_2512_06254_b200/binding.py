@@ -45,7 +45,7 @@ class toi_snapshot_info(C.Structure):
                 ("wsum", C.c_double), ("n_gridded", C.c_int64), ("n_off_grid", C.c_int64),
                 ("n_flagged", C.c_int64), ("ms_h2d", C.c_float), ("ms_planefit", C.c_float),
                 ("ms_weight", C.c_float), ("ms_grid", C.c_float), ("ms_fft", C.c_float),
-                ("ms_crop", C.c_float), ("ms_total", C.c_float), ("ms_clear", C.c_float)]
+                ("ms_crop", C.c_float), ("ms_total", C.c_float), ("ms_clear", C.c_float), ("ms_clear_density", C.c_float)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_ if k not in ("V", "sing")}

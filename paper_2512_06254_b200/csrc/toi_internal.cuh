@@ -188,12 +188,13 @@ inline cudaError_t launch_pdl(void (*kernel)(P...), dim3 grid, dim3 block, size_
 // rectangle starts on any column).
 constexpr int kClearTilesPerWarp = 4;
 __device__ __forceinline__ void clear_tiles_warp(float2 *__restrict__ grid, float *__restrict__ dens, int G,
-                                                 uint8_t *__restrict__ map, int tpr, long long n_tiles, long long t0, int lane)
+                                                 uint8_t *__restrict__ map, int tpr, long long n_tiles, long long t0, int lane,
+                                                 bool reset = true)
 {
     if (t0 >= n_tiles) return;
     const long long mine = t0 + lane;
     const bool dirty = lane < kClearTilesPerWarp && mine < n_tiles && map[mine] != 0;
-    if (dirty) map[mine] = 0;
+    if (dirty && reset) map[mine] = 0;     // reset == false: another clear launch follows on the same map
     unsigned todo = __ballot_sync(0xffffffffu, dirty);
     while (todo) {
         const int b = __ffs(todo) - 1;
@@ -336,7 +337,7 @@ void launch_grid_pair8(const Geometry &g, const Inputs &in, SnapState *st, const
 inline size_t grid_guard(int G) { return ((size_t)G + 8 + 31) / 32 * 32; }
 void launch_grid_pair8_cheb(const Geometry &g, const Inputs &in, SnapState *st, const float *d_density,
                             float2 *d_grid, uint8_t *tiles, int n_sms, const ChebArgs &cheb, cudaStream_t stream);
-void launch_clear_tiles(float2 *d_grid, float *d_density, int G, uint8_t *d_map, cudaStream_t stream);
+void launch_clear_tiles(float2 *d_grid, float *d_density, int G, uint8_t *d_map, cudaStream_t stream, bool reset_map = true);
 // hand-written pruned transform (k_fft.cu): rows through the tile map, then columns with the crop fused
 bool fft_custom_supported(int N, int G);
 void fft_twiddle_table(int G, float2 *host_out);

@@ -58,7 +58,8 @@ struct toi_plan {
     cudaEvent_t ev_done = nullptr;                       // end of the last imaging call, recorded only when the next
     cudaStream_t last_stream = nullptr;                  // call comes on ANOTHER stream than last_stream (an event
     bool have_last = false;                              // record between two kernels would break their launch overlap)
-    cudaEvent_t ev_clear0 = nullptr, ev_clear1 = nullptr;
+    cudaEvent_t ev_clear0 = nullptr, ev_clear1 = nullptr, ev_clear2 = nullptr;
+    bool timed_density_clear = false;  // the last timed call cleared the density map between ev_clear1 and ev_clear2
     float *d_images = nullptr;
     int ring_depth = 5;
     long long ring_pos = 0;                              // image ring only
@@ -199,6 +200,7 @@ int free_plan(toi_plan *p)
     if (p->ev_done) cudaEventDestroy(p->ev_done);
     if (p->ev_clear0) cudaEventDestroy(p->ev_clear0);
     if (p->ev_clear1) cudaEventDestroy(p->ev_clear1);
+    if (p->ev_clear2) cudaEventDestroy(p->ev_clear2);
     if (p->s_d2h) cudaStreamSynchronize(p->s_d2h);
     cudaFree(p->d_products);
     for (int k = 0; k < 2; ++k) {
@@ -297,11 +299,22 @@ int transform_and_clear(toi_plan *p, cudaStream_t stream, float2 *d_grid, uint8_
     // and 16384 the column pass has one CTA of 8-16 warps per SM and the clear is faster by itself).
     const bool clear_in_cols = p->fft_custom && !timed && g.G <= 4096;
     float *dens_to_clear = clear_density ? p->d_dens : nullptr;
-    if (!clear_in_cols) {
-        if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
+    if (!clear_in_cols && !timed) {
         launch_clear_tiles(d_grid, dens_to_clear, g.G, d_tiles, stream);
         ++*launches;
-        if (timed) CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
+    } else if (!clear_in_cols) {
+        // timed: the grid's clear (ms_clear, charged to the gridding) and the density map's
+        // (ms_clear_density, charged to the weighting) as two launches, each between its own events
+        CU_TRY(p, cudaEventRecord(p->ev_clear0, stream));
+        launch_clear_tiles(d_grid, nullptr, g.G, d_tiles, stream, dens_to_clear == nullptr);
+        ++*launches;
+        CU_TRY(p, cudaEventRecord(p->ev_clear1, stream));
+        p->timed_density_clear = dens_to_clear != nullptr;
+        if (dens_to_clear) {
+            launch_clear_tiles(nullptr, dens_to_clear, g.G, d_tiles, stream);
+            ++*launches;
+        }
+        CU_TRY(p, cudaEventRecord(p->ev_clear2, stream));
     }
     if (before_cols) CU_TRY(p, cudaStreamWaitEvent(stream, before_cols, 0));     // what still reads this lane's moment
     if (p->fft_custom) {
@@ -420,8 +433,10 @@ int read_info(toi_plan *p, cudaStream_t stream, toi_snapshot_info *info, bool ha
     cudaEventElapsedTime(&info->ms_grid, p->ev[EV_WEIGHT], p->ev[EV_GRID]);
     cudaEventElapsedTime(&info->ms_fft, p->ev[EV_GRID], p->ev[EV_FFT]);
     info->ms_clear = 0.0f;
+    info->ms_clear_density = 0.0f;
     if (cudaEventElapsedTime(&ms, p->ev_clear0, p->ev_clear1) == cudaSuccess) info->ms_clear = ms;
-    info->ms_fft -= info->ms_clear;
+    if (p->timed_density_clear && cudaEventElapsedTime(&ms, p->ev_clear1, p->ev_clear2) == cudaSuccess) info->ms_clear_density = ms;
+    info->ms_fft -= info->ms_clear + info->ms_clear_density;
     cudaEventElapsedTime(&info->ms_crop, p->ev[EV_FFT], p->ev[EV_CROP]);
     cudaEventElapsedTime(&info->ms_total, p->ev[EV_START], p->ev[EV_CROP]);
     cudaGetLastError();
@@ -564,6 +579,7 @@ int toi_plan_create(const toi_config *cfg, toi_plan **out)
     CREATE_TRY(cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming));
     CREATE_TRY(cudaEventCreate(&p->ev_clear0));
     CREATE_TRY(cudaEventCreate(&p->ev_clear1));
+    CREATE_TRY(cudaEventCreate(&p->ev_clear2));
     if (cfg->debug_keep_grid) {
         CREATE_TRY(cudaMalloc(&p->d_grid_keep, GG * sizeof(float2)));
         if (cfg->weighting == TOI_WEIGHT_UNIFORM) CREATE_TRY(cudaMalloc(&p->d_dens_keep, GG * sizeof(float)));

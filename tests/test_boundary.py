@@ -55,14 +55,14 @@ def test_struct_layouts_match_the_header(tmp_path):
         '#include <stdio.h>\n#include <stddef.h>\n#include "toi.h"\n'
         'int main(void){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n", sizeof(toi_3d_info), offsetof(toi_3d_info, ms_total), sizeof(toi_config), sizeof(toi_snapshot_info),'
         ' sizeof(toi_snapshot_buffers), sizeof(toi_stream_stats), offsetof(toi_config, chan_freq_hz),'
-        ' offsetof(toi_config, debug_keep_grid), offsetof(toi_snapshot_info, ms_clear), sizeof(toi_stream_output),'
+        ' offsetof(toi_config, debug_keep_grid), offsetof(toi_snapshot_info, ms_clear_density), sizeof(toi_stream_output),'
         ' offsetof(toi_stream_output, host_sink));return 0;}\n')
     exe = tmp_path / "layout"
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
     got = [int(x) for x in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
     want = [C.sizeof(toi.toi_3d_info), toi.toi_3d_info.ms_total.offset, C.sizeof(toi.toi_config), C.sizeof(toi.toi_snapshot_info), C.sizeof(toi.toi_snapshot_buffers),
             C.sizeof(toi.toi_stream_stats), toi.toi_config.chan_freq_hz.offset, toi.toi_config.debug_keep_grid.offset,
-            toi.toi_snapshot_info.ms_clear.offset, C.sizeof(toi.toi_stream_output), toi.toi_stream_output.host_sink.offset]
+            toi.toi_snapshot_info.ms_clear_density.offset, C.sizeof(toi.toi_stream_output), toi.toi_stream_output.host_sink.offset]
     assert got == want
 
 
