@@ -507,10 +507,12 @@ def run_e2e(r, args):
 # on `date`; this run cannot observe DRAM counters itself).  The sparse clear is a separate launch,
 # and most of the reductions stay in the 126 MB L2 until the FFT reads them, hence the small write figure.
 NCU_TRAFFIC = {
-    ("2", "uniform", "sliding"): {"bytes": 469522432 + 6200064, "source": "profiles/r2_k_grid_pair8_c2_uniform_full.txt",
-                                  "date": "round 2, commit 698d8db (the kernel this run times)"},
-    ("2", "natural", "sliding"): {"bytes": 458139648 + 6415872, "source": "profiles/r2_k_grid_pair8_c2_natural_full.txt",
-                                  "date": "round 2, commit d446d56 (the gridder is unchanged since, but for the programmatic-launch wait at its start)"},
+    ("2", "uniform", "sliding"): {"bytes": 471886080 + 5477120, "source": "profiles/r2_k_grid_pair8_c2_uniform_full.txt",
+                                  "date": "round 2, commit f42dad3 (the kernel this run times)"},
+    ("2", "natural", "sliding"): {"bytes": 460128000 + 5616128, "source": "profiles/r2_k_grid_pair8_c2_natural_full.txt",
+                                  "date": "round 2, commit f42dad3 (the kernel this run times)"},
+    ("4", "natural", "sliding"): {"bytes": 4047186000 + 106117376, "source": "profiles/r2_k_grid_pair8_c4_natural_full.txt",
+                                  "date": "round 2, commit f42dad3 (the kernel this run times)"},
     ("2", "uniform", "atomic"): {"bytes": 454289920 + 15841024, "source": "profiles/r2_k_grid_atomic_c2_uniform_full.txt",
                                  "date": "round 2, commit d446d56"},
 }

@@ -60,6 +60,8 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
 {
     static_assert(!(PIPE && CHEB), "the Chebyshev pass computes the cell in place");
     __shared__ uint4 s_rec[kWarps * kWarpQuads];
+    for (int i = threadIdx.x; i < kWarps * kWarpQuads; i += kWarps * 32) s_rec[i] = make_uint4(0u, 0u, 0u, 0u);
+    __syncthreads();
     pdl_wait();
     pdl_trigger();
     if (st->status != TOI_OK) return;
@@ -262,10 +264,8 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                         my_rec[4] = make_uint4(wu[4], wu[5], wu[6], wu[7]);
                     }
                 }
-                if (!valid) {
-                    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
-                    my_rec[1] = zero; my_rec[2] = zero; my_rec[3] = zero; my_rec[4] = zero;
-                }
+                // a record without a sample (flagged, off the grid, padding) keeps the taps its slot held
+                // before -- finite: the slots start at zero and only ever hold taps -- and has z = 0
                 float f = 1.0f;
                 if (has_d) {
                     // the density of a cell whose samples are all flagged is 0: never invert it
