@@ -179,7 +179,7 @@ k_grid_pair8(Geometry g, Inputs in, SnapState *__restrict__ st, const float *__r
                 const int bu = (iu - kH) & ~1, bv = (iv - kH) & ~1;
                 cl.key = cell_key(bu, bv);
                 cl.sh = (unsigned)((iu - kH) & 1) | ((unsigned)((iv - kH) & 1) << 1);
-                if (has_d) cl.dens = __ldg(Dc + ((long long)iv * G + iu));
+                if (has_d) cl.dens = __ldg(Dc + (iv * G + iu));      // |iv G + iu| < G^2 / 2 <= 2^29 (G <= 32768)
             } else {
                 cl.xu = cl.xv = 0.0f;          // taps stay finite whatever the coordinates were
                 if (count_rej) ++n_off;

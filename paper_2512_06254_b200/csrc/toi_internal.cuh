@@ -116,7 +116,8 @@ __device__ __forceinline__ size_t centre_index(int iu, int iv, int G)
 }
 
 // ---- data handling (G12/G13): select, never multiply by zero --------
-__device__ __forceinline__ bool weight_ok(float w) { return w > 0.0f && w <= 3.402823466e+38f; }
+// positive and finite, i.e. bit pattern in [1, 0x7f7fffff]: one integer compare instead of two float ones
+__device__ __forceinline__ bool weight_ok(float w) { return __float_as_uint(w) - 1u < 0x7f7fffffu; }
 
 // Effective per-hand weights of sample q (element offset o = q * n_p) and the Stokes-I weight.
 __device__ __forceinline__ void sample_weights(const Geometry &g, const Inputs &in, long long o, float &wa,
