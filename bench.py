@@ -507,12 +507,12 @@ def run_e2e(r, args):
 # on `date`; this run cannot observe DRAM counters itself).  The sparse clear is a separate launch,
 # and most of the reductions stay in the 126 MB L2 until the FFT reads them, hence the small write figure.
 NCU_TRAFFIC = {
-    ("2", "uniform", "sliding"): {"bytes": 471886080 + 5477120, "source": "profiles/r2_k_grid_pair8_c2_uniform_full.txt",
-                                  "date": "round 2, commit f42dad3 (the kernel this run times)"},
-    ("2", "natural", "sliding"): {"bytes": 460128000 + 5616128, "source": "profiles/r2_k_grid_pair8_c2_natural_full.txt",
-                                  "date": "round 2, commit f42dad3 (the kernel this run times)"},
-    ("4", "natural", "sliding"): {"bytes": 4047186000 + 106117376, "source": "profiles/r2_k_grid_pair8_c4_natural_full.txt",
-                                  "date": "round 2, commit f42dad3 (the kernel this run times)"},
+    ("2", "uniform", "sliding"): {"bytes": 471379456 + 6023680, "source": "profiles/r2_k_grid_pair8_c2_uniform_full.txt",
+                                  "date": "round 2, commit 88344db (the kernel this run times)"},
+    ("2", "natural", "sliding"): {"bytes": 459376640 + 5765376, "source": "profiles/r2_k_grid_pair8_c2_natural_full.txt",
+                                  "date": "round 2, commit 88344db (the kernel this run times)"},
+    ("4", "natural", "sliding"): {"bytes": 4022963000 + 106629376, "source": "profiles/r2_k_grid_pair8_c4_natural_full.txt",
+                                  "date": "round 2, commit 88344db (the kernel this run times)"},
     ("2", "uniform", "atomic"): {"bytes": 454289920 + 15841024, "source": "profiles/r2_k_grid_atomic_c2_uniform_full.txt",
                                  "date": "round 2, commit d446d56"},
 }
@@ -526,6 +526,7 @@ def main():
     from paper_2512_06254_b200 import binding as toi
     from paper_2512_06254_b200 import synth
     r = run_ours(args)
+    pcie_before = pinned_h2d_peak_gbs() if r["rank"] == 0 else 0.0
     e2e, stream_res = run_e2e(r, args)
     rank, world, wl, weighting = r["rank"], r["world"], r["wl"], r["weighting"]
     if world > 1:
@@ -555,7 +556,9 @@ def main():
     stages["ms_difference"] = round(r["extra"]["ms_difference"], 5)
     stages["difference_gbs"] = n2 * 12 / (r["extra"]["ms_difference_min"] * 1e-3) / 1e9
     stages["mode_3d"] = r["extra"].get("mode_3d")
-    pcie = pinned_h2d_peak_gbs()
+    # the pinned-copy rate of a fresh 1 GiB buffer varies by 2-4 % from allocation to allocation (where
+    # the pinned pages land): measured before and after the e2e / streamed runs, the better one is the roofline
+    pcie = max(pcie_before, pinned_h2d_peak_gbs())
     e2e["pcie_peak_gbs_measured"] = pcie
     e2e["pcie_frac"] = e2e["h2d_gbs_per_gpu"] / pcie
     if stream_res is not None:
