@@ -1,7 +1,7 @@
 // k_clear.cu -- sparse clear of the gridding grid and of the density map.
 //
-// A snapshot touches 2-3 % of the G x G cells (3091 of 16384 32x32 tiles at
-// config 2), so zero-filling the whole grid for every snapshot (134 MB of HBM writes at config 2,
+// A snapshot's windows reach a fraction of the G x G cells (a quarter of the 128 x 8-cell tiles at
+// config 2, about a tenth at config 4), so zero-filling the whole grid for every snapshot (134 MB of HBM writes at config 2,
 // 2.1 GB at config 4) is wasted traffic.  The gridder and the density pass mark the 128 x 8-cell
 // tiles they may write in a byte map; once the first FFT pass has read the grid (out of place, into
 // the FFT workspace) this kernel zeroes exactly those tiles again and resets the map, so the next

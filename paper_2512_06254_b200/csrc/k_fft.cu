@@ -2,8 +2,8 @@
 // (PAPER.md:301 names the inverse FFT as the heaviest stage).
 //   F[m][n] = sum_{y, x} grid[y][x] exp(+2 pi i (x n + y m) / G)       (array indices; the grid is stored
 //   centred, which multiplies F by (-1)^(n + m): undone where the image is written, as in k_correct_crop)
-// Only the N columns n and N rows m the crop keeps are ever needed, and only 2-3 % of the grid is
-// non-zero.  Two kernels, both built on the shared-memory FFT of fft_smem.cuh:
+// Only the N columns n and N rows m the crop keeps are ever needed, and most of the grid is
+// zero (three quarters of its tiles at config 2, about nine tenths at config 4).  Two kernels, both built on the shared-memory FFT of fft_smem.cuh:
 //   k_fft_rows   one CTA per grid row: the row is read THROUGH THE TILE MAP of the sparse clear (tiles
 //                the gridder did not mark are known to be zero and are not read: 36 MB instead of
 //                134 MB at config 2) straight into the first stage's registers, transformed along x,
