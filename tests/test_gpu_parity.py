@@ -285,6 +285,12 @@ def test_calls_without_info_give_the_same_image(weighting):
         img, info, _ = gi.image()
         _assert_image(img, img_o, "timed call after untimed ones")
         assert info["ms_grid"] > 0.0 and info["ms_fft"] > 0.0
+        # a timed call clears the grid and the density map with two launches, each between its own events
+        assert info["ms_clear"] > 0.0
+        assert (info["ms_clear_density"] > 0.0) == (weighting == "uniform")
+        img, rc_g = gi.image_untimed()
+        assert rc_g == 0
+        _assert_image(img, img_o, "untimed call after a timed one")
 
 
 def test_edge_non_default_grid_size():
